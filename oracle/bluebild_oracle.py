@@ -1,0 +1,182 @@
+"""ORACLE — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+A plain, slow, fp64 CPU implementation of the Bluebild Standard Synthesis path, written from
+/root/reference/PAPER.md (arXiv 2310.09200) and from nothing else. Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may
+import it. It shares no code with ``paper_2310_09200_b200`` (the CUDA path) and never imports it.
+
+Functions and the passage each follows:
+
+===================  ==========================================================================
+``gram``             Eq. 11 Psi_pq = sinc(2 ||b_pq||), b = (f/c)(x_p - x_q), sinc
+                     normalized; Eq. 24 G = W^H Psi W.
+``geig``             Eq. 13 V alpha = lambda G alpha, solved as G = L L^H,
+                     C = L^-1 S L^-H, Hermitian eig of C, alpha = L^-H Q  (so alpha^H G alpha = I).
+``select``           Alg. 1 line 4: keep the N_eig largest eigenvalues.
+``level_weights``    Alg. 1 lines 7-8: D[l,k] = d_f(lambda_k) if lambda_k in
+                     [min_l, max_l] else 0; LSQ filter d = lambda, STD filter d = 1.
+``synth``            Alg. 2 + Alg. 1 line 9 (C++: oracle/synth.cpp).
+``brute``            the literal definition, tiny inputs (C++: oracle/brute.cpp).
+``collect``          Alg. 1 end to end.
+===================  ==========================================================================
+
+Library primitives used as steps: numpy.linalg.cholesky, numpy.linalg.eigh, numpy.linalg.solve,
+numpy.sinc. Pins: tests/test_oracle_pins.py (P1-P6, I1-I8 of DESIGN.md). Parity unpinned: none.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liboracle.so")
+_SOURCES = ["synth.cpp", "brute.cpp"]
+_lib = None
+
+C_LIGHT = 299792458.0  # m/s; wavelength = c / f (reading Q3: PAPER.md:117 prints "f/c")
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/*.cpp into oracle/liboracle.so (g++ -O2, no fast-math)."""
+    srcs = [os.path.join(_HERE, s) for s in _SOURCES]
+    if (not force and os.path.exists(_LIB_PATH)
+            and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(s) for s in srcs)):
+        return _LIB_PATH
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", _LIB_PATH] + srcs
+    subprocess.run(cmd, check=True)
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB_PATH)
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_synth.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int64,
+                                     dp, ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int,
+                                     dp, ctypes.c_int64, ctypes.c_double, dp, ctypes.c_int]
+        lib.oracle_synth.restype = ctypes.c_int
+        lib.oracle_brute.argtypes = lib.oracle_synth.argtypes[:-1]
+        lib.oracle_brute.restype = ctypes.c_int
+        lib.oracle_hardware_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def hardware_threads() -> int:
+    return int(_load().oracle_hardware_threads())
+
+
+def _f(a, dtype):
+    return np.asfortranarray(np.asarray(a, dtype=dtype))
+
+
+def _dptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+# ---------------------------------------------------------------------------------- glue steps
+def gram(xyz, W, wavelength):
+    """Eq. 11 + Eq. 24. xyz (n_ant,3) metres; W (n_ant,n_beam) complex or None (identity)."""
+    xyz = np.asarray(xyz, dtype=np.float64)
+    diff = xyz[:, None, :] - xyz[None, :, :]
+    dist = np.sqrt(np.sum(diff * diff, axis=-1))           # ||x_p - x_q||
+    psi = np.sinc(2.0 * dist / wavelength)                 # sinc(2 ||b_pq||), np.sinc is normalized
+    if W is None:
+        return psi.astype(np.complex128)
+    W = np.asarray(W, dtype=np.complex128)
+    return W.conj().T @ psi @ W
+
+
+def geig(S, G):
+    """Eq. 13: S v = lambda G v with V^H G V = I. Returns (lambda ascending, V columns)."""
+    S = np.asarray(S, dtype=np.complex128)
+    G = np.asarray(G, dtype=np.complex128)
+    S = 0.5 * (S + S.conj().T)                             # reading Q10
+    G = 0.5 * (G + G.conj().T)
+    L = np.linalg.cholesky(G)                              # G = L L^H
+    Y = np.linalg.solve(L, S)                              # L^-1 S
+    C = np.linalg.solve(L, Y.conj().T).conj().T            # L^-1 S L^-H
+    C = 0.5 * (C + C.conj().T)
+    lam, Q = np.linalg.eigh(C)
+    V = np.linalg.solve(L.conj().T, Q)                     # L^-H Q
+    return lam, V
+
+
+def select(lam, V, n_eig):
+    """Alg. 1 line 4: N_eig largest eigenvalues (by signed value, reading Q6), descending."""
+    order = np.argsort(lam, kind="stable")[::-1][:n_eig]
+    return lam[order], V[:, order]
+
+
+def level_weights(lam, intervals, filt="lsq"):
+    """D[l,k] for closed intervals [min_l, max_l] (reading Q7), LSQ (d = lambda) or STD (d = 1)."""
+    lam = np.asarray(lam, dtype=np.float64)
+    intervals = np.asarray(intervals, dtype=np.float64).reshape(-1, 2)
+    inside = (lam[None, :] >= intervals[:, :1]) & (lam[None, :] <= intervals[:, 1:])
+    d = lam if filt == "lsq" else np.ones_like(lam)
+    return np.where(inside, d[None, :], 0.0)
+
+
+# ---------------------------------------------------------------------------------- synthesis
+def synth(B, D, xyz, pix, wavelength, img=None, n_threads=0):
+    """I_l(r_j) += sum_k D[l,k] |sum_i conj(B_ik) exp(+j 2 pi <p_i,r_j>/lambda_w)|^2 (Alg. 2)."""
+    B = _f(B, np.complex128)
+    D = _f(np.atleast_2d(D), np.float64)
+    xyz = _f(xyz, np.float64)
+    pix = _f(pix, np.float64)
+    n_ant, n_eig = B.shape
+    n_levels = D.shape[0]
+    n_pix = pix.shape[0]
+    assert D.shape[1] == n_eig and xyz.shape == (n_ant, 3) and pix.shape[1] == 3
+    if img is None:
+        img = np.zeros((n_levels, n_pix), dtype=np.float64)
+    assert img.shape == (n_levels, n_pix) and img.dtype == np.float64 and img.flags.c_contiguous
+    rc = _load().oracle_synth(n_ant, n_eig, n_levels, n_pix, _dptr(B), max(n_ant, 1),
+                              _dptr(D), max(n_levels, 1), _dptr(xyz), max(n_ant, 1), _dptr(pix),
+                              max(n_pix, 1), float(wavelength), _dptr(img), int(n_threads))
+    if rc != 0:
+        raise ValueError("oracle_synth: invalid arguments")
+    return img
+
+
+def brute(B, D, xyz, pix, wavelength):
+    """Literal triple sum with the exponential in the innermost loop (tiny inputs only)."""
+    B = _f(B, np.complex128)
+    D = _f(np.atleast_2d(D), np.float64)
+    xyz = _f(xyz, np.float64)
+    pix = _f(pix, np.float64)
+    n_ant, n_eig = B.shape
+    n_levels, n_pix = D.shape[0], pix.shape[0]
+    img = np.zeros((n_levels, n_pix), dtype=np.float64)
+    _load().oracle_brute(n_ant, n_eig, n_levels, n_pix, _dptr(B), max(n_ant, 1),
+                         _dptr(D), max(n_levels, 1), _dptr(xyz), max(n_ant, 1), _dptr(pix),
+                         max(n_pix, 1), float(wavelength), _dptr(img))
+    return img
+
+
+# ---------------------------------------------------------------------------------- Alg. 1
+def eig_stage(S, W, xyz, wavelength, n_eig, gram_identity=False):
+    """Alg. 1 lines 2-4 and U = W alpha. Returns (lambda desc (n_eig,), B (n_ant,n_eig))."""
+    n_ant = np.asarray(xyz).shape[0]
+    if gram_identity:                                       # G := I special case
+        G = np.eye(np.asarray(S).shape[0], dtype=np.complex128)
+    else:
+        G = gram(xyz, W, wavelength)
+    lam, V = geig(S, G)
+    lam, V = select(lam, V, n_eig)
+    B = V if W is None else np.asarray(W, dtype=np.complex128) @ V
+    assert B.shape[0] == n_ant
+    return lam, B
+
+
+def collect(S, W, xyz, wavelength, n_eig, intervals, pix, img=None, filt="lsq",
+            gram_identity=False, n_threads=0):
+    """Algorithm 1 for one time step / channel; accumulates into img."""
+    lam, B = eig_stage(S, W, xyz, wavelength, n_eig, gram_identity)
+    D = level_weights(lam, intervals, filt)
+    return synth(B, D, xyz, pix, wavelength, img=img, n_threads=n_threads)
