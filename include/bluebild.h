@@ -1,0 +1,126 @@
+/* bluebild.h — C ABI of the B200-native Bluebild Standard Synthesizer (libbluebild_b200.so).
+ *
+ * Method: arXiv 2310.09200 (BIPP), /root/reference/PAPER.md. Interface follows the paper's
+ * "Context + imaging handle + collect per time step" design (Table 1
+ * PAPER.md:250-258, Algorithm 1 line 1 PAPER.md:285): column-major inputs, host or device.
+ *
+ * Conventions for EVERY entry point
+ *   - Every data pointer may be a HOST or a DEVICE pointer (classified with
+ *     cudaPointerGetAttributes). Host buffers are snapshotted before the call returns; device
+ *     buffers are read in stream order on the context stream and must stay valid until work
+ *     already enqueued on that stream has consumed them (i.e. until bb_synth_flush/get returns
+ *     or the stream is synchronised).
+ *   - The caller owns all buffers; the library never frees or retains caller memory.
+ *   - Return value: BB_OK or an error code; no exception crosses the ABI. All arguments are
+ *     validated before any launch, so a failed call leaves the level images unchanged and the
+ *     handle usable.
+ *   - All matrices are column-major with an explicit leading dimension (in elements).
+ *   - Complex single precision is interleaved (re, im) pairs of float (bb_c32).
+ *   - There is no CPU fallback: without a CUDA device bb_ctx_create fails with BB_ECUDA.
+ */
+#ifndef BLUEBILD_B200_H
+#define BLUEBILD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bb_ctx bb_ctx;     /* device, stream, library handles, scratch ("Context") */
+typedef struct bb_synth bb_synth; /* StandardSynthesis imaging handle                   */
+typedef struct { float re, im; } bb_c32;
+
+enum {
+  BB_OK = 0,
+  BB_EINVAL = 1,       /* bad argument (null pointer, non-positive size, ld too small, n_eig > n_beam ...) */
+  BB_EALLOC = 2,       /* host or device allocation failed */
+  BB_ECUDA = 3,        /* CUDA runtime / library error (no device, launch failure) */
+  BB_ENOTPOSDEF = 4,   /* Gram matrix not positive definite (Cholesky failed) */
+  BB_ENOCONV = 5,      /* eigensolver did not converge */
+  BB_ESTATE = 6,       /* call not valid in the handle's state */
+  BB_EUNSUPPORTED = 7  /* variant / size not supported by this build */
+};
+
+enum {
+  BB_VARIANT_FP32 = 0,    /* FP32 CUDA-core synthesizer (FFMA2), fp64-reduced phases          */
+  BB_VARIANT_TF32X3 = 1   /* tcgen05 tensor-core synthesizer, 3xTF32 split, fp32 accumulation */
+};
+
+/* ---- context ------------------------------------------------------------------------------
+ * device: CUDA ordinal. cuda_stream: a cudaStream_t (may be NULL = default stream) on which all
+ * work of handles created from this context is enqueued. */
+int bb_ctx_create(int device, void* cuda_stream, bb_ctx** out);
+int bb_ctx_destroy(bb_ctx* ctx);
+
+/* ---- imaging handle -----------------------------------------------------------------------
+ * pix: X_pix of Table 1: n_pix x 3 pixel unit vectors, column-major with leading
+ * dimension ld_pix >= n_pix, float64, same sky-fixed frame as the antenna positions.
+ * n_levels: number of eigenvalue intervals N_i (1..BB_MAX_LEVELS). Images start at zero. */
+#define BB_MAX_LEVELS 32
+#define BB_MAX_BEAMS 512
+int bb_synth_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pix, int n_levels,
+                    int variant, bb_synth** out);
+int bb_synth_destroy(bb_synth* s);
+int bb_synth_reset(bb_synth* s); /* drop pending collects and zero the level images */
+
+/* ---- collect: Algorithm 1 for one time step / channel -------------------
+ * G = W^H Psi W with Psi_pq = sinc(2 |x_p - x_q| / wavelength) (Eq. 11, 24; normalized sinc);
+ * S v = lambda G v with V^H G V = I (Eq. 13); keep the n_eig largest lambda (Alg. 1 l.4);
+ * B = W V; D[l,k] = lambda_k if intervals[l,0] <= lambda_k <= intervals[l,1] else 0 (closed
+ * intervals, tested independently: overlap counts twice, uncovered eigenvalues are dropped);
+ * then bb_synth_collect_eig. Glue runs in fp64 on the device.
+ *   W   n_ant x n_beam complex64, ld ldw; NULL means identity (requires n_beam == n_ant)
+ *   S   n_beam x n_beam complex64 Hermitian, full storage, ld lds (used as (S+S^H)/2)
+ *   xyz n_ant x 3 float64 metres, ld ldxyz (P_icrs of Table 1)
+ *   intervals n_levels x 2 float64, ld ld_int: column 0 = min, column 1 = max
+ * Limits: 1 <= n_eig <= n_beam <= BB_MAX_BEAMS, n_ant >= 1, wavelength > 0. */
+int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength,
+                     const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz,
+                     int ldxyz, const double* intervals, int ld_int);
+
+/* ---- collect_eig: the hot path only (Algorithm 2 + Alg. 1 line 9, Eq. 15, 20) ---------------
+ * I_l(r_j) += sum_k D[l,k] | sum_i conj(B_ik) exp(+j 2 pi <xyz_i, r_j> / wavelength) |^2
+ *   B   n_ant x n_eig complex64 (= W V), ld ldb
+ *   D   n_levels x n_eig float32 weights, ld ldd
+ *   xyz n_ant x 3 float64, ld ldxyz
+ * The call enqueues a small preparation kernel and queues the collect; the fused synthesizer
+ * kernel runs when the queue is full, on bb_synth_flush, or on bb_synth_get, looping over all
+ * queued collects inside one launch (every time step and band). */
+int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wavelength, const bb_c32* B,
+                         int ldb, const float* D, int ldd, const double* xyz, int ldxyz);
+
+/* Launch the synthesizer over all queued collects now (asynchronous; does not synchronise). */
+int bb_synth_flush(bb_synth* s);
+
+/* Copy level image `level` (n_pix float32, pixel order of pix) to out (host or device).
+ * Flushes pending collects and synchronises the context stream. Images are plain sums over
+ * collects (Alg. 1 line 9: "+="; no division by the number of collects). */
+int bb_synth_get(bb_synth* s, int level, float* out);
+
+/* Device-measured times (CUDA events, ms) accumulated since create/reset; any may be NULL. */
+int bb_synth_timings(bb_synth* s, double* gram_ms, double* eig_ms, double* prep_ms, double* synth_ms);
+
+/* Number of kernels this handle has launched since create/reset. */
+int64_t bb_synth_launches(bb_synth* s);
+
+/* ---- eigen stage alone (Alg. 1 lines 2-4), for parameter estimation ----
+ * lambda_out: n_eig float64 eigenvalues, descending. B_out (may be NULL): n_ant x n_eig
+ * complex64, ld ldb_out. Same argument rules as bb_synth_collect. Synchronises the stream. */
+int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W,
+           int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz, double* lambda_out,
+           bb_c32* B_out, int ldb_out);
+
+/* ---- peak probes (measurement support) --------------------------------
+ * kind: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2), 2 = MUFU sin+cos, 3 = DFMA. Runs a register-only
+ * loop on every SM and returns operations per second in *ops_per_s (FMA counted as 1 op per
+ * lane; kind 1 counts 2 per lane-instruction) and the kernel time in *ms. */
+int bb_probe_peak(bb_ctx* ctx, int kind, double* ops_per_s, double* ms);
+
+const char* bb_status_string(int status);
+const char* bb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLUEBILD_B200_H */

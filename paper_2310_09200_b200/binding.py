@@ -1,0 +1,211 @@
+"""Thin ctypes binding of libbluebild_b200.so (include/bluebild.h). Argument marshalling only:
+every step of the path runs in the library's CUDA kernels; there is no CPU fallback, and a missing
+library or a missing GPU raises.
+
+Matrices are column-major. Host arguments are numpy arrays (converted to Fortran
+order if needed). Device arguments are ``DeviceMatrix`` objects (a torch CUDA tensor holding the
+column-major data) — torch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbluebild_b200.so")
+
+BB_OK = 0
+VARIANT_FP32 = 0
+VARIANT_TF32X3 = 1
+_VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, 0: 0, 1: 1}
+
+EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
+           "bb_synth_collect", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
+           "bb_synth_launches", "bb_eig", "bb_probe_peak", "bb_status_string", "bb_version"]
+
+_lib = None
+
+
+class BluebildError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = _lib.bb_status_string(code).decode() if _lib is not None else "?"
+        super().__init__("%s failed: [%d] %s" % (where, code, msg))
+
+
+def load_library(path: str = LIB_PATH):
+    """Load the C-ABI library; raises if it has not been built (python -m paper_2310_09200_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise ImportError("CUDA extension %s is missing: run `python -m paper_2310_09200_b200.build` "
+                          "(there is no CPU fallback)" % path)
+    lib = ctypes.CDLL(path)
+    vp, i32, i64, f64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
+    pp = ctypes.POINTER(ctypes.c_void_p)
+    pd = ctypes.POINTER(ctypes.c_double)
+    sig = {
+        "bb_ctx_create": ([i32, vp, pp], i32),
+        "bb_ctx_destroy": ([vp], i32),
+        "bb_synth_create": ([vp, i64, vp, i64, i32, i32, pp], i32),
+        "bb_synth_destroy": ([vp], i32),
+        "bb_synth_reset": ([vp], i32),
+        "bb_synth_collect": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32], i32),
+        "bb_synth_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
+        "bb_synth_flush": ([vp], i32),
+        "bb_synth_get": ([vp, i32, vp], i32),
+        "bb_synth_timings": ([vp, pd, pd, pd, pd], i32),
+        "bb_synth_launches": ([vp], i64),
+        "bb_eig": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, vp, i32], i32),
+        "bb_probe_peak": ([vp, i32, pd, pd], i32),
+        "bb_status_string": ([i32], ctypes.c_char_p),
+        "bb_version": ([], ctypes.c_char_p),
+    }
+    for name, (args, res) in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes, fn.restype = args, res
+    _lib = lib
+    return lib
+
+
+def _check(code, where):
+    if code != BB_OK:
+        raise BluebildError(code, where)
+
+
+class DeviceMatrix:
+    """A column-major (rows x cols) matrix in device memory, backed by a torch CUDA tensor of shape
+    (cols, rows) (its row-major storage is the column-major matrix; ld = rows)."""
+
+    def __init__(self, tensor, rows, cols):
+        assert tensor.is_cuda and tensor.is_contiguous()
+        self.tensor, self.rows, self.cols, self.ld = tensor, rows, cols, rows
+
+    @classmethod
+    def from_numpy(cls, a, dtype, device="cuda:0"):
+        import torch
+        a = np.asarray(a, dtype=dtype)
+        if a.ndim == 1:
+            a = a[:, None]
+        t = torch.from_numpy(np.ascontiguousarray(a.T)).to(device)
+        return cls(t, a.shape[0], a.shape[1])
+
+    @property
+    def ptr(self):
+        return self.tensor.data_ptr()
+
+
+def _marshal(a, dtype, keep):
+    """-> (pointer as int, rows, cols, ld). numpy -> Fortran-ordered host buffer (kept alive in `keep`)."""
+    if a is None:
+        return None, 0, 0, 1
+    if isinstance(a, DeviceMatrix):
+        return a.ptr, a.rows, a.cols, a.ld
+    arr = np.asarray(a, dtype=dtype)
+    if arr.ndim == 1:
+        arr = arr[:, None]
+    arr = np.asfortranarray(arr)
+    keep.append(arr)
+    return arr.ctypes.data, arr.shape[0], arr.shape[1], max(arr.shape[0], 1)
+
+
+class Context:
+    """bb_ctx: device + stream + library handles (PAPER.md:262 'Context')."""
+
+    def __init__(self, device: int = 0, stream=None):
+        lib = load_library()
+        h = ctypes.c_void_p()
+        sp = None
+        if stream is not None:
+            sp = ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+        _check(lib.bb_ctx_create(int(device), sp, ctypes.byref(h)), "bb_ctx_create")
+        self._h, self._stream, self.device = h, stream, device
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.bb_ctx_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def probe_peak(self, kind: int):
+        ops, ms = ctypes.c_double(), ctypes.c_double()
+        _check(_lib.bb_probe_peak(self._h, kind, ctypes.byref(ops), ctypes.byref(ms)), "bb_probe_peak")
+        return ops.value, ms.value
+
+    def eig(self, S, W, xyz, wavelength, n_eig, want_B=True):
+        """Alg. 1 lines 2-4: (lambda desc float64 (n_eig,), B complex64 (n_ant, n_eig))."""
+        keep = []
+        Sp, n_beam, _, lds = _marshal(S, np.complex64, keep)
+        Wp, _, _, ldw = _marshal(W, np.complex64, keep)
+        Xp, n_ant, _, ldx = _marshal(xyz, np.float64, keep)
+        lam = np.zeros(n_eig, dtype=np.float64)
+        B = np.zeros((n_ant, n_eig), dtype=np.complex64, order="F") if want_B else None
+        _check(_lib.bb_eig(self._h, n_ant, n_beam, n_eig, float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
+                           lam.ctypes.data, B.ctypes.data if want_B else None, max(n_ant, 1)), "bb_eig")
+        return lam, B
+
+
+class StandardSynthesis:
+    """bb_synth: the imaging handle (Algorithm 1)."""
+
+    def __init__(self, ctx: Context, pix, n_levels: int, variant="fp32"):
+        keep = []
+        Pp, n_pix, c, ld = _marshal(pix, np.float64, keep)
+        assert c == 3, "pix must be (n_pix, 3)"
+        h = ctypes.c_void_p()
+        _check(_lib.bb_synth_create(ctx._h, n_pix, Pp, ld, int(n_levels), _VARIANTS[variant], ctypes.byref(h)),
+               "bb_synth_create")
+        self._h, self.ctx, self.n_pix, self.n_levels = h, ctx, n_pix, n_levels
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.bb_synth_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def reset(self):
+        _check(_lib.bb_synth_reset(self._h), "bb_synth_reset")
+
+    def collect(self, S, W, xyz, wavelength, n_eig, intervals):
+        keep = []
+        Sp, n_beam, _, lds = _marshal(S, np.complex64, keep)
+        Wp, _, _, ldw = _marshal(W, np.complex64, keep)
+        Xp, n_ant, _, ldx = _marshal(xyz, np.float64, keep)
+        Ip, _, _, ldi = _marshal(intervals, np.float64, keep)
+        _check(_lib.bb_synth_collect(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
+                                     Ip, ldi), "bb_synth_collect")
+
+    def collect_eig(self, B, D, xyz, wavelength):
+        keep = []
+        Bp, n_ant, n_eig, ldb = _marshal(B, np.complex64, keep)
+        Dp, _, _, ldd = _marshal(D, np.float32, keep)
+        Xp, _, _, ldx = _marshal(xyz, np.float64, keep)
+        _check(_lib.bb_synth_collect_eig(self._h, n_ant, n_eig, float(wavelength), Bp, ldb, Dp, ldd, Xp, ldx),
+               "bb_synth_collect_eig")
+
+    def flush(self):
+        _check(_lib.bb_synth_flush(self._h), "bb_synth_flush")
+
+    def get(self, level: int, out=None):
+        """Level image as float32 (n_pix,). `out` may be a numpy array or a torch CUDA tensor."""
+        if out is None:
+            out = np.empty(self.n_pix, dtype=np.float32)
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        _check(_lib.bb_synth_get(self._h, int(level), ptr), "bb_synth_get")
+        return out
+
+    def images(self):
+        return np.stack([self.get(l) for l in range(self.n_levels)])
+
+    def timings(self):
+        v = [ctypes.c_double() for _ in range(4)]
+        _check(_lib.bb_synth_timings(self._h, *[ctypes.byref(x) for x in v]), "bb_synth_timings")
+        return dict(gram_ms=v[0].value, eig_ms=v[1].value, prep_ms=v[2].value, synth_ms=v[3].value)
+
+    def launches(self) -> int:
+        return int(_lib.bb_synth_launches(self._h))

@@ -1,0 +1,95 @@
+// Internal declarations shared by the translation units of libbluebild_b200.so.
+// Nothing here is part of the ABI (include/bluebild.h is) and nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstddef>
+#include <vector>
+
+#include "../../include/bluebild.h"
+
+#define BB_CUDA(call)                                         \
+  do {                                                        \
+    cudaError_t err__ = (call);                               \
+    if (err__ != cudaSuccess) { bb_note_cuda_error(err__, #call, __FILE__, __LINE__); return BB_ECUDA; } \
+  } while (0)
+
+void bb_note_cuda_error(cudaError_t err, const char* what, const char* file, int line);
+
+// ------------------------------------------------------------------------------------------
+// Packed per-collect operand layout of the FP32 synthesizer.
+//   eigenpairs are padded to n_slabs * GC * KT; antennas to n_chunks * AC.
+//   collect buffer = [slab][chunk]{ B part: AC x (GC*KT/2) float4 (br_2q, br_2q+1, bi_2q, bi_2q+1)
+//                                   P part: AC x 4 double (p'_x, p'_y, p'_z, 0) }
+//   weights        = [level][n_eig_pad] float
+// B already carries the per-antenna constant phase exp(-j 2 pi <p'_i, r_c>) (centring identity).
+struct Fp32Plan {
+  int KT;        // eigenpairs per thread (template parameter of the kernel)
+  int PT;        // pixels per thread
+  int GC;        // eigen-groups per CTA (CTA = 128 threads = GC groups of 128/GC threads)
+  int AC;        // antennas per staged chunk
+  int n_slabs;   // ceil(n_eig / (GC*KT))
+  int n_chunks;  // ceil(n_ant / AC)
+  int n_eig_pad; // n_slabs * GC * KT
+  int n_ant_pad; // n_chunks * AC
+  size_t chunk_bytes;    // AC * (GC*KT*8 + 32)
+  size_t collect_bytes;  // n_slabs * n_chunks * chunk_bytes
+  size_t weight_floats;  // n_levels * n_eig_pad
+};
+
+Fp32Plan bb_fp32_plan(int n_ant, int n_eig, int n_levels);
+
+// Packed operand layout of the tensor-core (3xTF32) synthesizer; see kernels_tc.cu.
+struct TcPlan {
+  int AC;            // antennas per K-chunk (K = 2*AC real columns per pass)
+  int NB;            // N of the MMA = 2 * n_eig_pad_slab (Re | Im' halves)
+  int n_slabs, n_chunks, n_eig_pad, n_ant_pad, eig_per_slab;
+  size_t chunk_bytes;    // B_hi + B_lo tiles in UMMA canonical layout + p' block
+  size_t collect_bytes;
+  size_t weight_floats;
+};
+TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels);
+
+struct PrepArgs {
+  const bb_c32* B; int ldb;           // device
+  const float* D; int ldd;            // device
+  const double* xyz; int ldxyz;       // device
+  int n_ant, n_eig, n_levels;
+  double wavelength;
+  double rc[3];
+  unsigned char* packed;              // device: collect buffer
+  float* weights;                     // device: [level][n_eig_pad]
+};
+
+int bb_launch_prep_fp32(const Fp32Plan& plan, const PrepArgs& a, cudaStream_t st);
+int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st);
+
+struct SynthArgs {
+  const double* rprime; int64_t n_pix; int64_t pix_stride;  // r' SoA: [3][pix_stride]
+  const unsigned char* packed; size_t packed_stride;       // queued collects, contiguous slots
+  const float* weights; size_t weight_stride;              // floats per slot
+  int n_collects, n_levels;
+  float* img; int64_t img_stride;                          // [level][img_stride]
+};
+// returns number of kernels launched in *launches
+int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
+int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
+
+// pixel preparation: bounding-box centre r_c and r' = r - r_c (SoA fp64)
+int bb_pixels_prepare(const double* pix_dev, int64_t n_pix, int64_t ld_pix, double* rprime,
+                      int64_t pix_stride, double rc_out[3], cudaStream_t st);
+
+// glue (Alg. 1 lines 2-4) — glue.cu
+struct GlueWork;
+int bb_glue_create(GlueWork** out);
+void bb_glue_destroy(GlueWork* g);
+// Computes lambda (n_eig, descending, device fp64) and B = W V (n_ant x n_eig complex64, device,
+// ld n_ant). W/S/xyz are device pointers. Timed with the given events (may be null).
+int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, double wavelength,
+                const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
+                double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
+                cudaEvent_t ev_eig0, cudaEvent_t ev_eig1);
+int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int,
+                            int n_levels, float* D_dev, int ldd, cudaStream_t st);
+
+int bb_probe_run(int kind, int sm_count, cudaStream_t st, double* ops_per_s, double* ms);

@@ -1,0 +1,147 @@
+"""GPU edge cases of the hot path through the C ABI: ragged tiles, odd eigen counts, many levels,
+negative weights, queue overflow, determinism, argument validation."""
+import numpy as np
+import pytest
+
+from helpers import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = ["fp32"]
+
+
+@pytest.fixture(scope="module")
+def bb():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2310_09200_b200 import binding
+    binding.load_library()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(bb):
+    return bb.Context(0)
+
+
+def random_case(seed, n_ant, n_eig, n_levels, n_pix, extent=3000.0, fov=0.25, signed=False):
+    rng = np.random.default_rng(seed)
+    B = ((rng.normal(size=(n_ant, n_eig)) + 1j * rng.normal(size=(n_ant, n_eig))) / np.sqrt(n_ant)).astype(np.complex64)
+    D = rng.uniform(0.1, 3.0, size=(n_levels, n_eig)) * (rng.random((n_levels, n_eig)) < 0.5)
+    if signed:
+        D *= rng.choice([-1.0, 1.0], size=D.shape)
+    xyz = rng.uniform(-extent, extent, size=(n_ant, 3)) + np.array([6.1e6, -2.3e5, 1.7e6])   # far from the origin
+    lm = rng.uniform(-fov, fov, size=(n_pix, 2))
+    c = np.array([0.3, -0.5, np.sqrt(1 - 0.34)])
+    e1 = np.cross(c, [0, 0, 1.0]); e1 /= np.linalg.norm(e1)
+    e2 = np.cross(c, e1)
+    pix = lm[:, :1] * e1 + lm[:, 1:] * e2 + np.sqrt(1 - np.sum(lm * lm, axis=1))[:, None] * c
+    return dict(B=np.asfortranarray(B), D=np.asfortranarray(D.astype(np.float32)), xyz=np.asfortranarray(xyz),
+                pix=np.asfortranarray(pix), wavelength=2.7)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("n_ant,n_eig,n_levels,n_pix", [
+    (1, 1, 1, 1), (16, 8, 2, 1000), (37, 5, 3, 513), (50, 13, 4, 777), (33, 16, 1, 257), (70, 31, 5, 300),
+    (64, 33, 2, 129), (40, 64, 8, 255), (48, 65, 3, 200), (20, 130, 2, 150), (24, 7, 32, 100)])
+def test_shapes_ragged_and_padded(bb, ctx, oracle, variant, n_ant, n_eig, n_levels, n_pix):
+    c = random_case(1000 + n_ant + n_eig, n_ant, n_eig, n_levels, n_pix, signed=True)
+    ref = oracle.synth(c["B"], c["D"], c["xyz"], c["pix"], c["wavelength"])
+    s = bb.StandardSynthesis(ctx, c["pix"], n_levels, variant)
+    s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    got = s.images()
+    scale = np.max(np.abs(ref))
+    for l in range(n_levels):       # signed weights: measure against the overall peak
+        assert np.max(np.abs(got[l] - ref[l])) <= 1e-4 * scale, (l, np.max(np.abs(got[l] - ref[l])) / scale)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_leading_dimensions_and_device_pointers(bb, ctx, oracle, variant):
+    import torch
+    c = random_case(7, 21, 6, 2, 300)
+    ref = oracle.synth(c["B"], c["D"], c["xyz"], c["pix"], c["wavelength"])
+    # padded leading dimensions on the device side
+    def padded(a, dtype, extra):
+        rows, cols = a.shape
+        t = torch.zeros((cols, rows + extra), dtype=dtype, device="cuda:0")
+        t[:, :rows] = torch.from_numpy(np.ascontiguousarray(a.T)).to("cuda:0")
+        m = bb.DeviceMatrix(t, rows, cols)
+        m.ld = rows + extra
+        return m
+    s = bb.StandardSynthesis(ctx, padded(c["pix"], torch.float64, 11), 2, variant)
+    s.collect_eig(padded(c["B"], torch.complex64, 3), padded(c["D"], torch.float32, 5), padded(c["xyz"], torch.float64, 2),
+                  c["wavelength"])
+    out = torch.empty(300, dtype=torch.float32, device="cuda:0")
+    got = np.stack([s.get(l, out).cpu().numpy().copy() for l in range(2)])
+    assert_parity(got, ref, "ld")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_queue_overflow_additivity_reset_and_determinism(bb, ctx, oracle, variant):
+    c = random_case(11, 18, 8, 2, 400)
+    rng = np.random.default_rng(5)
+    ref = np.zeros((2, 400))
+    s = bb.StandardSynthesis(ctx, c["pix"], 2, variant)
+    cases = []
+    for e in range(70):             # more collects than the queue holds: several launches accumulate
+        B = np.asfortranarray((c["B"] * np.exp(1j * rng.uniform(0, 6.28, size=8))).astype(np.complex64))
+        xyz = np.asfortranarray(c["xyz"] + rng.normal(0, 5.0, size=c["xyz"].shape))
+        cases.append((B, xyz))
+        oracle.synth(B, c["D"], xyz, c["pix"], c["wavelength"], img=ref)
+        s.collect_eig(B, c["D"], xyz, c["wavelength"])
+    a = s.images()
+    assert_parity(a, ref, "70 collects")
+    s.reset()
+    assert np.all(s.images() == 0)
+    for B, xyz in cases:
+        s.collect_eig(B, c["D"], xyz, c["wavelength"])
+    assert np.array_equal(s.images(), a)        # bit-exact run to run
+    # mixed shapes flush the queue and keep accumulating
+    c2 = random_case(12, 9, 3, 2, 400)
+    s.collect_eig(c2["B"], c2["D"], c2["xyz"], c2["wavelength"])
+    oracle.synth(c2["B"], c2["D"], c2["xyz"], c["pix"], c2["wavelength"], img=ref)
+    assert_parity(s.images(), ref, "mixed shapes")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_zero_weights_give_exact_zero_and_nonnegativity(bb, ctx, variant):
+    c = random_case(13, 30, 12, 3, 500)
+    c["D"][1, :] = 0
+    s = bb.StandardSynthesis(ctx, c["pix"], 3, variant)
+    s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    img = s.images()
+    assert np.all(img[1] == 0) and np.all(img >= 0) and img[0].max() > 0
+
+
+def test_argument_validation(bb, ctx):
+    c = random_case(14, 10, 4, 2, 50)
+    with pytest.raises(bb.BluebildError) as e:
+        bb.StandardSynthesis(ctx, c["pix"], 0)
+    assert e.value.code == 1
+    with pytest.raises(bb.BluebildError):
+        bb.StandardSynthesis(ctx, c["pix"], 33)
+    s = bb.StandardSynthesis(ctx, c["pix"], 2)
+    with pytest.raises(bb.BluebildError) as e:
+        s.collect_eig(c["B"], c["D"], c["xyz"], -1.0)
+    assert e.value.code == 1
+    with pytest.raises(bb.BluebildError):
+        s.get(2)
+    with pytest.raises(bb.BluebildError):        # n_eig > n_beam
+        s.collect(np.eye(4, dtype=np.complex64), None, c["xyz"][:4], 2.0, 5, np.array([[0.0, 1.0], [1.0, 2.0]]))
+    # a failed call leaves the images unchanged and the handle usable
+    assert np.all(s.images() == 0)
+    s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    assert s.images().max() > 0
+    # Gram not positive definite: two coincident antennas
+    xyz = np.asfortranarray(np.zeros((4, 3)))
+    with pytest.raises(bb.BluebildError) as e:
+        s.collect(np.eye(4, dtype=np.complex64), None, xyz, 2.0, 2, np.array([[0.0, 1.0], [1.0, 2.0]]))
+    assert e.value.code == 4
+
+
+def test_empty_image(bb, ctx):
+    s = bb.StandardSynthesis(ctx, np.zeros((0, 3)), 1)
+    c = random_case(15, 5, 2, 1, 4)
+    s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    s.flush()
+    assert s.get(0).shape == (0,)
