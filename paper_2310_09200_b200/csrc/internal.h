@@ -28,6 +28,7 @@ struct Fp32Plan {
   int PT;        // pixels per thread
   int GC;        // eigen-groups per CTA (CTA = 128 threads = GC groups of 128/GC threads)
   int AC;        // antennas per staged chunk
+  int MINB;      // __launch_bounds__ min CTAs per SM the kernel is compiled for
   int n_slabs;   // ceil(n_eig / (GC*KT))
   int n_chunks;  // ceil(n_ant / AC)
   int n_eig_pad; // n_slabs * GC * KT

@@ -20,6 +20,12 @@
 //     per launch (8*L bytes per pixel per launch).
 #include "internal.h"
 #include <cuda.h>
+#include <cstdio>
+#include <cstdlib>
+
+#ifndef BB_ORDER
+#define BB_ORDER 0
+#endif
 
 namespace {
 
@@ -68,8 +74,8 @@ __device__ __forceinline__ void phase_cs(double px, double py, double pz, double
 }
 
 // ---------------------------------------------------------------------------- synthesizer
-template <int KT, int PT, int GC>
-__global__ void __launch_bounds__(kThreads, 2)
+template <int KT, int PT, int GC, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB)
 synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                   const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                   const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset,
@@ -153,21 +159,43 @@ synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_
 #pragma unroll
           for (int p = 0; p < PT; ++p) phase_cs(pp.x, pp.y, pp.z, rx[p], ry[p], rz[p], cn[p], snn[p]);
         }
-        // a2: 4 FFMA2 per (pixel, eigen-pair)
+        // a2: 4 FFMA2 per (pixel, eigen-pair). Order matters: an FFMA2 reads 5 registers (scalar, pair,
+        // accumulator pair) and the register file delivers 2 per bank per FFMA2 slot, so consecutive
+        // FFMA2 must share an operand through the operand-reuse cache.
+#if BB_ORDER == 0
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
           const float4 b = brow[(size_t)i * ROW4 + q];
           const float2 br = make_float2(b.x, b.y), bi = make_float2(b.z, b.w);
 #pragma unroll
+          for (int p = 0; p < PT; ++p) re[p][q] = __ffma2_rn(make_float2(cs[p], cs[p]), br, re[p][q]);
+#pragma unroll
+          for (int p = 0; p < PT; ++p) im[p][q] = __ffma2_rn(make_float2(-sn[p], -sn[p]), br, im[p][q]);
+#pragma unroll
+          for (int p = 0; p < PT; ++p) re[p][q] = __ffma2_rn(make_float2(sn[p], sn[p]), bi, re[p][q]);
+#pragma unroll
+          for (int p = 0; p < PT; ++p) im[p][q] = __ffma2_rn(make_float2(cs[p], cs[p]), bi, im[p][q]);
+        }
+#else
+        {
+          float4 b[NQ];
+#pragma unroll
+          for (int q = 0; q < NQ; ++q) b[q] = brow[(size_t)i * ROW4 + q];
+#pragma unroll
           for (int p = 0; p < PT; ++p) {
             const float2 cc = make_float2(cs[p], cs[p]), ss = make_float2(sn[p], sn[p]);
             const float2 ns = make_float2(-sn[p], -sn[p]);
-            re[p][q] = __ffma2_rn(cc, br, re[p][q]);
-            re[p][q] = __ffma2_rn(ss, bi, re[p][q]);
-            im[p][q] = __ffma2_rn(cc, bi, im[p][q]);
-            im[p][q] = __ffma2_rn(ns, br, im[p][q]);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) re[p][q] = __ffma2_rn(cc, make_float2(b[q].x, b[q].y), re[p][q]);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) im[p][q] = __ffma2_rn(cc, make_float2(b[q].z, b[q].w), im[p][q]);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) re[p][q] = __ffma2_rn(ss, make_float2(b[q].z, b[q].w), re[p][q]);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) im[p][q] = __ffma2_rn(ns, make_float2(b[q].x, b[q].y), im[p][q]);
           }
         }
+#endif
 #pragma unroll
         for (int p = 0; p < PT; ++p) { cs[p] = cn[p]; sn[p] = snn[p]; }
       }
@@ -271,12 +299,12 @@ prep_fp32_kernel(PrepArgs a, int KT, int GC, int AC, int n_slabs, int n_chunks, 
   }
 }
 
-template <int KT, int PT, int GC>
+template <int KT, int PT, int GC, int MINB>
 int launch_variant(const Fp32Plan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   constexpr int TG = kThreads / GC;
   const size_t smem = align_up((size_t)kStages * plan.chunk_bytes, 128) +
                       (size_t)a.n_levels * PT * kThreads * 4 + 2 * (size_t)a.n_levels * GC * KT * 4 + kStages * 8 + 16;
-  auto kern = synth_fp32_kernel<KT, PT, GC>;
+  auto kern = synth_fp32_kernel<KT, PT, GC, MINB>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + TG * PT - 1) / (TG * PT);
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
@@ -300,7 +328,12 @@ Fp32Plan bb_fp32_plan(int n_ant, int n_eig, int n_levels) {
   else if (n_eig <= 32) { p.KT = 32; p.PT = 2; p.GC = 1; }
   else if (n_eig <= 64) { p.KT = 32; p.PT = 2; p.GC = 2; }
   else { p.KT = 32; p.PT = 2; p.GC = 4; }
+  p.MINB = 2;
   p.AC = 32;
+  if (const char* e = getenv("BB_FP32_CFG")) {   // tuning experiments: "KT,PT,GC,MINB,AC"
+    int kt, pt, gc, mb, ac;
+    if (sscanf(e, "%d,%d,%d,%d,%d", &kt, &pt, &gc, &mb, &ac) == 5) { p.KT = kt; p.PT = pt; p.GC = gc; p.MINB = mb; p.AC = ac; }
+  }
   const int per_slab = p.GC * p.KT;
   p.n_slabs = (n_eig + per_slab - 1) / per_slab;
   p.n_chunks = (n_ant + p.AC - 1) / p.AC;
@@ -326,10 +359,12 @@ int bb_launch_prep_fp32(const Fp32Plan& plan, const PrepArgs& a, cudaStream_t st
 int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
   *launches = 0;
   if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
-  if (plan.KT == 8) return launch_variant<8, 4, 1>(plan, a, st, launches);
-  if (plan.KT == 12) return launch_variant<12, 4, 1>(plan, a, st, launches);
-  if (plan.KT == 16) return launch_variant<16, 4, 1>(plan, a, st, launches);
-  if (plan.GC == 1) return launch_variant<32, 2, 1>(plan, a, st, launches);
-  if (plan.GC == 2) return launch_variant<32, 2, 2>(plan, a, st, launches);
-  return launch_variant<32, 2, 4>(plan, a, st, launches);
+#define BB_CASE(kt, pt, gc, mb) \
+  if (plan.KT == kt && plan.PT == pt && plan.GC == gc && plan.MINB == mb) return launch_variant<kt, pt, gc, mb>(plan, a, st, launches);
+  BB_CASE(8, 4, 1, 2) BB_CASE(12, 4, 1, 2) BB_CASE(16, 4, 1, 2)
+  BB_CASE(32, 2, 1, 2) BB_CASE(32, 2, 2, 2) BB_CASE(32, 2, 4, 2)
+  BB_CASE(16, 2, 4, 4) BB_CASE(16, 2, 4, 3) BB_CASE(32, 1, 2, 4) BB_CASE(32, 1, 2, 3) BB_CASE(16, 2, 2, 4) BB_CASE(16, 2, 1, 4)
+  BB_CASE(32, 2, 2, 3) BB_CASE(16, 4, 4, 2) BB_CASE(8, 4, 1, 4) BB_CASE(12, 2, 1, 4) BB_CASE(8, 2, 1, 4)
+#undef BB_CASE
+  return BB_EUNSUPPORTED;
 }
