@@ -70,6 +70,17 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tc_commit_mc(uint64_t* bar, uint16_t mask) {   // same barrier offset in every CTA of the mask
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)), "h"(mask) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_mc(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint16_t mask) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;" ::"r"(
+                   smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "h"(mask) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 // D[tmem] (+)= A[tmem] * B[smem desc]; kind::tf32, cta_group::1
@@ -120,11 +131,15 @@ __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) 
 // ---------------------------------------------------------------------------- synthesizer
 // Chunk in global/shared memory (N = 2 NE rows, kK columns):
 //   [ B_hi : (kK/4) core columns x (N/8) row groups x (8 rows x 16 B) ][ B_lo : same ][ p' : kAC x 4 double ]
+// With CS > 1 the CTAs of a cluster consume the same B chunks: each CTA fetches 1/CS of every chunk and
+// multicasts it to all CTAs of the cluster (L2 -> SM traffic / CS); a stage is reused only after the MMAs of
+// ALL CTAs of the cluster have read it (tcgen05.commit multicast onto every CTA's b_empty, count CS).
+template <int CS>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                 const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                 const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset, int NE,
-                int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride) {
+                int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride, int dbg) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int N = 2 * NE;
   const uint32_t half_bytes = (uint32_t)kK * N * 4;                 // one of B_hi / B_lo
@@ -146,7 +161,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   if (tid == 0) {
-    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 1); }
+    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], CS); }
     for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[s], kProducerThreads / 32); mbar_init(&a_empty[s], 1); }
     mbar_init(d_full, 1);
     mbar_init(d_empty, kProducerThreads / 32);
@@ -159,6 +174,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   for (int i = tid; i < n_levels * kProducerThreads; i += kThreadsTC) lev[i] = 0.f;
   tc_fence_before();
   __syncthreads();
+  if (CS > 1) cluster_sync_all();          // every CTA's barriers are initialised before any remote arrive / copy
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const int total = n_collects * n_chunks;
@@ -190,8 +206,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
 #pragma unroll
           for (int a = 0; a < 8; ++a) {
             const double4 pp = prow[h * 8 + a];
-            float cs, sn;
-            phase_cs(pp.x, pp.y, pp.z, rx, ry, rz, cs, sn);
+            float cs = 0.5f, sn = 0.25f;
+            if (!(dbg & 1)) phase_cs(pp.x, pp.y, pp.z, rx, ry, rz, cs, sn);
             split_tf32(cs, hi[2 * a], lo[2 * a]);
             split_tf32(sn, hi[2 * a + 1], lo[2 * a + 1]);
           }
@@ -267,11 +283,11 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
               for (int kk = 0; kk < kK / 8; ++kk) {
                 const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
                 const uint64_t bd = make_b_desc((pass == 2 ? b_lo : b_hi) + kk * 2 * lbo, lbo, sbo);
-                mma_tf32_ts(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
+                if (!(dbg & 2)) mma_tf32_ts(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
               }
           }
           tc_commit(&a_empty[sa]);
-          tc_commit(&b_empty[sb]);
+          if (CS > 1) tc_commit_mc(&b_empty[sb], (uint16_t)((1u << CS) - 1)); else tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
         }
       }
@@ -285,12 +301,18 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         const int e = n / n_chunks, c = n - e * n_chunks;
         const unsigned char* src = packed + (size_t)e * packed_stride + slab_offset + (size_t)c * chunk_bytes;
         mbar_expect_tx(&b_full[sb], chunk_bytes);
-        bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
+        if (CS > 1) {
+          const uint32_t part = chunk_bytes / CS, off = cluster_rank() * part;
+          bulk_g2s_mc(stage_base + (size_t)sb * chunk_bytes + off, src + off, part, &b_full[sb], (uint16_t)((1u << CS) - 1));
+        } else {
+          bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
+        }
       }
     }
   }
   tc_fence_before();
   __syncthreads();
+  if (CS > 1) cluster_sync_all();          // no CTA exits while a peer may still multicast into it
   if (warp == 8) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols));
@@ -395,21 +417,39 @@ int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
   return BB_OK;
 }
 
-int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
-  *launches = 0;
-  if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
+template <int CS>
+static int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches, int dbg) {
   const int NE = plan.eig_per_slab;
   const size_t smem = align_up((size_t)kSB * plan.chunk_bytes, 1024) + (size_t)a.n_levels * kProducerThreads * 4 +
                       2 * (size_t)a.n_levels * NE * 4 + (2 * kSB + 2 * kSA + 2) * 8 + 16 + 1024;
-  BB_CUDA(cudaFuncSetAttribute(synth_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int64_t tiles = (a.n_pix + kProducerThreads - 1) / kProducerThreads;
+  auto kern = synth_tc_kernel<CS>;
+  BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int64_t tiles = (a.n_pix + kProducerThreads - 1) / kProducerThreads;
+  tiles = (tiles + CS - 1) / CS * CS;     // whole clusters; surplus CTAs own no pixel but take part in the B exchange
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)tiles);
+  cfg.blockDim = dim3(kThreadsTC);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
-    synth_tc_kernel<<<(unsigned)tiles, kThreadsTC, smem, st>>>(
-        a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride, (size_t)slab * plan.n_chunks * plan.chunk_bytes,
-        a.weights, a.weight_stride, plan.n_eig_pad, slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img,
-        a.img_stride);
-    BB_CUDA(cudaGetLastError());
+    BB_CUDA(cudaLaunchKernelEx(&cfg, kern, a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
+                               (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights, a.weight_stride, plan.n_eig_pad,
+                               slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img, a.img_stride, dbg));
     ++*launches;
   }
   return BB_OK;
+}
+
+int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
+  *launches = 0;
+  if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
+  const int dbg = getenv("BB_TC_DEBUG") ? atoi(getenv("BB_TC_DEBUG")) : 0;        // timing experiments only
+  const int cs = getenv("BB_TC_CLUSTER") ? atoi(getenv("BB_TC_CLUSTER")) : 2;
+  if (cs == 1) return launch_tc<1>(plan, a, st, launches, dbg);
+  if (cs == 4) return launch_tc<4>(plan, a, st, launches, dbg);
+  return launch_tc<2>(plan, a, st, launches, dbg);
 }
