@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — synthesizer throughput of the B200-native Bluebild Standard Synthesizer.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fp32|tf32x3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fp32|tf32x3|fp16x3]
                     [--impl ours|reference] [--probe]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: all collects of
@@ -314,7 +314,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if args.variant == "fp32" else "tf32x3", "data": "synthetic",
+        "dtype": {"fp32": "f32", "tf32x3": "tf32x3", "fp16x3": "fp16x3"}[args.variant], "data": "synthetic",
         "config": {"workload": "config %d: %s" % (c.idx, c.name), "n_ant": c.n_ant, "n_beam": c.n_beam, "n_eig": c.n_eig,
                    "n_levels": L, "n_pix": c.n_pix, "n_collects": c.n_collects, "variant": args.variant,
                    "parallelism": "replicas x%d (no collective)" % world,
@@ -334,14 +334,15 @@ def run_ours(args):
     bound = "alu"
     if args.variant != "fp32":
         mp = measured_peaks()
-        peak = 0.5 * mp["bf16_tflops"]              # dense TF32 = 1/2 of dense bf16 (guide's nominal ratio)
+        # dense FP16 = dense bf16; dense TF32 = 1/2 of it (guide's nominal ratio)
+        peak = mp["bf16_tflops"] * (1.0 if args.variant == "fp16x3" else 0.5)
         bound = "tensor"
     line["roofline"] = {"bound": bound, "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s",
                         "frac": achieved_tflops / peak, "traffic": None,
                         "kernel": "synth_fp32_kernel" if args.variant == "fp32" else "synth_tc_kernel",
                         "flops_per_launch": flops_per_launch, "avg_launch_ms": avg_launch_ms,
                         "peak_basis": ("148 SM x 128 FP32 lanes x 2 x 1.965 GHz (derived, DESIGN.md)" if bound == "alu" else
-                                       "0.5 x measured bf16 burst (MEASURED_PEAKS.json); useful flops = 8/term, issued = 24/term")}
+                                       ("1.0" if args.variant == "fp16x3" else "0.5") + " x measured bf16 burst (MEASURED_PEAKS.json); useful flops = 8/term, issued = 24/term")}
     if clocks.get("sm_mhz"):
         line["roofline"]["frac_at_observed_clock"] = achieved_tflops / (peak * clocks["sm_mhz"] / SM_MAX_MHZ) if bound == "alu" else None
     if args.probe:

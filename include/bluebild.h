@@ -44,7 +44,9 @@ enum {
 
 enum {
   BB_VARIANT_FP32 = 0,    /* FP32 CUDA-core synthesizer (FFMA2), fp64-reduced phases          */
-  BB_VARIANT_TF32X3 = 1   /* tcgen05 tensor-core synthesizer, 3xTF32 split, fp32 accumulation */
+  BB_VARIANT_TF32X3 = 1,  /* tcgen05 tensor-core synthesizer, 3xTF32 split, fp32 accumulation */
+  BB_VARIANT_FP16X3 = 2   /* same with the operands split into FP16 pairs (same 11-bit significand as TF32,
+                             B columns pre-scaled by powers of two): twice the tensor rate            */
 };
 
 /* ---- context ------------------------------------------------------------------------------

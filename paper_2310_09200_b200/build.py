@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libbluebild_b200.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC = os.path.join(CUDA_HOME, "bin", "nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-diag-suppress", "177"]
+         "-Xcompiler", "-fPIC", "-diag-suppress", "177"] + os.environ.get("BB_NVCC_EXTRA", "").split()
 
 
 def _deps():

@@ -1,4 +1,4 @@
-// tcgen05 (3xTF32) tensor-core variant of the fused Standard Synthesizer (sm_100a).
+// tcgen05 tensor-core variants of the fused Standard Synthesizer (sm_100a): 3xTF32 and 3xFP16 split precision.
 //
 // Same rows a1-a4 as kernels_fp32.cu (Alg. 2, Eq. 15, Eq. 20, Alg. 1 l.9), but the
 // contraction runs on the 5th-generation tensor cores as a REAL GEMM:
@@ -9,34 +9,56 @@
 //     A[j,(i,cos)] = cos phi_ij, A[j,(i,sin)] = sin phi_ij
 //     Bop[(Re,k),(i,cos)] = b_re, Bop[(Re,k),(i,sin)] = b_im, Bop[(Im',k),(i,cos)] = b_im, Bop[(Im',k),(i,sin)] = -b_re
 //   so Re E_kj = sum_i (c b_re + s b_im), Im' E_kj = sum_i (c b_im - s b_re): 8 real flops per term.
-// Split precision: x = hi + lo, hi = x with the 13 low mantissa bits cleared (exactly a TF32), lo = x - hi
-// (exact); D += A_hi B_hi + A_lo B_hi + A_hi B_lo with fp32 accumulation in TMEM (lo*lo ~ 2^-22 dropped).
+// Split precision: x = hi + lo with hi, lo in the 11-bit-significand tensor format (TF32, or FP16 with the
+// B columns pre-scaled by a power of two into FP16's range and the weights D[l,k] divided by its square);
+// D += A_hi B_hi + A_lo B_hi + A_hi B_lo with fp32 accumulation in TMEM (lo*lo ~ 2^-22 dropped).
+// FP16 carries the same significand as TF32 at twice the tensor rate and half the operand bytes.
 //
-// CTA = 2 pixel tiles of 128 (256 pixels), 320 threads, 1 CTA per SM, all 512 TMEM columns:
-//   warps 0-7  producers + epilogue: phase generator (fp64 fixed-point reduction, MUFU), hi/lo split,
+// Phase generator (a1) WITHOUT fp64: DFMA shares hardware with the tensor pipe on B200 (a dependent DFMA
+// chain runs 2.6x slower while tcgen05.mma is streaming, and the 3-DFMA reduction of kernels_fp32.cu made
+// the producers serialise with the MMAs), so the range reduction is done in exact integer arithmetic:
+//     p'_d = IH_d 2^-8 + PL_d      (IH = rint(p' 2^8) int32, |PL| <= 2^-9; per antenna, written by prep)
+//     r'_d = JH_d 2^-24 + RL_d     (JH = rint(r' 2^24) int32, |RL| <= 2^-25; per pixel, once per thread)
+//     frac(<p', r'>) = [ sum_d IH_d * JH_d mod 2^32 ] 2^-32  +  sum_d ( PH_d RL_d + PL_d r'_d )      (turns)
+//   three wrapping 32-bit IMADs give the large part exactly; the small part (< 2^-6 turns) is 6 fp32 FMAs.
+//   The 32-bit fraction is converted with the 1.5*2^23 magic-add (no I2F on the MUFU pipe), then MUFU.SIN/COS.
+//
+// CTA = 2 pixel tiles of 128 (256 pixels), 576 threads, 1 CTA per SM, all 512 TMEM columns:
+//   warps 0-15 producers + epilogue (two groups alternating chunks): phase generator, hi/lo split,
 //              tcgen05.st of their A rows straight into TMEM (A operand from TMEM: no smem round trip);
-//              after the last chunk of a collect: tcgen05.ld of D, |E|^2, level weights, level sums.
-//   warp 8     one elected thread issues tcgen05.mma.cta_group::1.kind::tf32 (A from TMEM, B from smem
-//              descriptors) and tcgen05.commit to the stage / accumulator mbarriers; owns TMEM alloc.
-//   warp 9     one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
+//              per collect: tcgen05.ld of D, |E|^2, level weights, level sums.
+//   warp 16    one elected thread issues tcgen05.mma.cta_group::1 (A from TMEM, B from smem descriptors)
+//              and tcgen05.commit to the stage / accumulator mbarriers; owns TMEM alloc.
+//   warp 17    one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
 //              layout, written by prep_tc_kernel) global -> shared with cp.async.bulk on mbarriers.
 #include "internal.h"
+#include <cuda_fp16.h>
 #include <cstdio>
 #include <cstdlib>
 
 namespace {
 
-constexpr int kProducerThreads = 256;
-constexpr int kThreadsTC = 320;
+constexpr int kTilePixels = 256;        // pixels per CTA (2 tiles of 128 TMEM lanes)
+constexpr int kProducerWarps = 16;      // 2 groups x 2 tiles x 4 lane quadrants
+constexpr int kThreadsTC = (kProducerWarps + 2) * 32;
 constexpr int kAC = 16;                 // antennas per chunk
-constexpr int kK = 2 * kAC;             // tf32 K-columns per chunk and pass
-constexpr int kSA = 2;                  // A stages (TMEM)
-constexpr int kSB = 4;                  // B stages (shared memory)
+constexpr int kK = 2 * kAC;             // K-columns (cos, sin per antenna) per chunk and pass
+constexpr int kRec = 48;                // bytes of one antenna record {IH[3],0 | 2pi PH[3],0 | 2pi PL[3],0}
 constexpr int kMaxNE = 64;              // eigenpairs per slab
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t
-constexpr uint32_t kColA = 256;         // A of stage s, tile t at kColA + 128 s + 64 t (+0 hi, +32 lo)
-constexpr double kMagic = 1572864.0;    // 1.5 * 2^20 (see kernels_fp32.cu)
+constexpr uint32_t kColA = 256;         // A stages
+constexpr float kTwoPi = 6.283185307179586f;
+
+template <int MODE> struct Cfg;
+template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (tile, hi|lo)
+  static constexpr int kElem = 4, kSA = 2, kSB = 4, kColsHalf = kK, kMmaPerPass = kK / 8;
+  static constexpr uint32_t kFmt = 2;   // instruction-descriptor operand format: TF32
+};
+template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one antenna share a 32-bit column
+  static constexpr int kElem = 2, kSA = 4, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
+  static constexpr uint32_t kFmt = 0;   // F16
+};
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -70,26 +92,17 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tc_commit_mc(uint64_t* bar, uint16_t mask) {   // same barrier offset in every CTA of the mask
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)), "h"(mask) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s_mc(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint16_t mask) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;" ::"r"(
-                   smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "h"(mask) : "memory");
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// D[tmem] (+)= A[tmem] * B[smem desc]; kind::tf32, cta_group::1
-__device__ __forceinline__ void mma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
-      : "memory");
+// D[tmem] (+)= A[tmem] * B[smem desc]; cta_group::1
+template <int MODE>
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  if (MODE == BB_TC_TF32)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+  else
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 // shared-memory matrix descriptor: K-major, no swizzle; core matrix = 8 rows x 16 bytes, contiguous 128 B
 __device__ __forceinline__ uint64_t make_b_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -115,11 +128,30 @@ __device__ __forceinline__ void tmem_ld8(uint32_t addr, float (&v)[8]) {
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
-__device__ __forceinline__ void phase_cs(double px, double py, double pz, double rx, double ry, double rz, float& c, float& s) {
-  double t = fma(px, rx, kMagic);
-  t = fma(py, ry, t);
-  t = fma(pz, rz, t);
-  const float x = (float)__double2loint(t) * (6.283185307179586f / 4294967296.0f);
+// Per-pixel constants of the integer phase generator.
+struct PixelSplit {
+  int jx, jy, jz;        // JH = rint(r' 2^24)
+  float lx, ly, lz;      // RL = r' - JH 2^-24
+  float fx, fy, fz;      // r' rounded to fp32
+};
+__device__ __forceinline__ void split_pixel(double r, int& j, float& l, float& f) {
+  const double s = rint(r * 16777216.0);
+  j = (int)s;
+  l = (float)(r - s * (1.0 / 16777216.0));
+  f = (float)r;
+}
+// cos / sin of 2 pi <p', r'> from one antenna record (three 16-byte words in shared memory).
+__device__ __forceinline__ void phase_cs(const int4& ih, const float4& ph, const float4& pl, const PixelSplit& q, float& c, float& s) {
+  const uint32_t fr = (uint32_t)ih.x * (uint32_t)q.jx + (uint32_t)ih.y * (uint32_t)q.jy + (uint32_t)ih.z * (uint32_t)q.jz;
+  float ls = ph.x * q.lx;
+  ls = fmaf(ph.y, q.ly, ls);
+  ls = fmaf(ph.z, q.lz, ls);
+  ls = fmaf(pl.x, q.fx, ls);
+  ls = fmaf(pl.y, q.fy, ls);
+  ls = fmaf(pl.z, q.fz, ls);
+  // signed fraction of a turn, top 23 bits, as an exactly representable float (magic add, no I2F)
+  const float f = __int_as_float(0x4B400000 + ((int)fr >> 9)) - 12582912.0f;
+  const float x = fmaf(f, kTwoPi / 8388608.0f, ls);        // radians in (-pi - eps, pi + eps)
   c = __cosf(x);
   s = __sinf(x);
 }
@@ -127,33 +159,58 @@ __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) 
   hi = __float_as_uint(x) & 0xFFFFE000u;
   lo = __float_as_uint(x - __uint_as_float(hi));
 }
+// (cos, sin) -> packed FP16 pairs: hi = rn16(x), lo = rn16(x - hi); K order (cos, sin) = (low, high) half
+__device__ __forceinline__ void split_f16(float c, float s, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(c, s);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(c - hf.x, s - hf.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
+#ifdef BB_TC_TRACE
+__device__ long long g_trace[4][128][4];
+__device__ __forceinline__ long long clk64() { long long c; asm volatile("mov.u64 %0, %%clock64;" : "=l"(c)); return c; }
+#define TR(role, slot) do { if (blockIdx.x == 0 && n < 128) g_trace[role][n][slot] = clk64(); } while (0)
+#else
+#define TR(role, slot) do { } while (0)
+#endif
 
 // ---------------------------------------------------------------------------- synthesizer
-// Chunk in global/shared memory (N = 2 NE rows, kK columns):
-//   [ B_hi : (kK/4) core columns x (N/8) row groups x (8 rows x 16 B) ][ B_lo : same ][ p' : kAC x 4 double ]
-// With CS > 1 the CTAs of a cluster consume the same B chunks: each CTA fetches 1/CS of every chunk and
-// multicasts it to all CTAs of the cluster (L2 -> SM traffic / CS); a stage is reused only after the MMAs of
-// ALL CTAs of the cluster have read it (tcgen05.commit multicast onto every CTA's b_empty, count CS).
-template <int CS>
+// Chunk in global/shared memory (N = 2 NE rows, kK columns of kElem bytes):
+//   [ B_hi : (kK*kElem/16) core columns x (N/8) row groups x (8 rows x 16 B) ][ B_lo : same ][ kAC antenna records ]
+//
+// Producer warps: w = 0..15; lane quadrant w & 3 (the TMEM lanes a warp may touch), tile (w >> 2) & 1,
+// group w >> 3. Group g produces the chunks n with (n & 1) == g, so each SM sub-partition always holds four
+// producer warps in different phases of their chunk (latency hiding) while per-chunk fixed costs stay
+// amortised over 16 antennas. The epilogue of collect e is deferred until both groups have produced their
+// first chunk of collect e+1, so the tensor pipe restarts on ready operands as soon as D is released;
+// the two groups split the eigenpair columns of D between them.
+template <int MODE>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                 const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                 const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset, int NE,
                 int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride, int dbg) {
+  using C = Cfg<MODE>;
+  constexpr int kSA = C::kSA, kSB = C::kSB;
+  constexpr uint32_t kColsStage = 4 * C::kColsHalf;                 // 2 tiles x (hi | lo)
+  static_assert(kColA + kSA * kColsStage <= kTmemCols, "TMEM budget");
+  static_assert(kSA % 2 == 0, "chunk parity must map to a fixed set of A stages");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int N = 2 * NE;
-  const uint32_t half_bytes = (uint32_t)kK * N * 4;                 // one of B_hi / B_lo
-  const uint32_t chunk_bytes = 2 * half_bytes + kAC * 32;
+  const uint32_t half_bytes = (uint32_t)kK * N * C::kElem;          // one of B_hi / B_lo
+  const uint32_t chunk_bytes = 2 * half_bytes + kAC * kRec;
   const uint32_t lbo = (uint32_t)(N / 8) * 128, sbo = 128;
 
   unsigned char* stage_base = smem_raw;
-  float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [L][256]
-  float* dsm = lev + (size_t)n_levels * kProducerThreads;                                        // [2][L][NE]
+  float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [2 groups][L][256]
+  float* dsm = lev + 2 * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
   uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + 2 * (size_t)n_levels * NE);
   uint64_t* b_full = bars;                 // [kSB]
-  uint64_t* b_empty = bars + kSB;          // [kSB]
-  uint64_t* a_full = bars + 2 * kSB;       // [kSA]
-  uint64_t* a_empty = a_full + kSA;        // [kSA]
+  uint64_t* b_empty = b_full + kSB;        // [kSB]
+  uint64_t* a_full = b_empty + kSB;        // [kSA][2 tiles]
+  uint64_t* a_empty = a_full + 2 * kSA;    // [kSA]
   uint64_t* d_full = a_empty + kSA;
   uint64_t* d_empty = d_full + 1;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
@@ -161,191 +218,270 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   if (tid == 0) {
-    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], CS); }
-    for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[s], kProducerThreads / 32); mbar_init(&a_empty[s], 1); }
+    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 1); }
+    for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 1); }
     mbar_init(d_full, 1);
-    mbar_init(d_empty, kProducerThreads / 32);
+    mbar_init(d_empty, kProducerWarps);
     fence_barrier_init();
   }
-  if (warp == 8) {
+  if (warp == kProducerWarps) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
   }
-  for (int i = tid; i < n_levels * kProducerThreads; i += kThreadsTC) lev[i] = 0.f;
+  for (int i = tid; i < 2 * n_levels * kTilePixels; i += kThreadsTC) lev[i] = 0.f;
+  for (int i = tid; i < n_levels * NE; i += kThreadsTC) {          // weights of collect 0
+    const int l = i / NE, k = i - l * NE;
+    dsm[i] = weights[(size_t)l * n_eig_pad + eig_offset + k];
+  }
   tc_fence_before();
   __syncthreads();
-  if (CS > 1) cluster_sync_all();          // every CTA's barriers are initialised before any remote arrive / copy
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const int total = n_collects * n_chunks;
 
-  if (warp < 8) {
+  if (warp < kProducerWarps) {
     // ===================== producers / epilogue: one pixel (TMEM lane) per thread =====================
-    const int tile = warp >> 2;
+    const int group = warp >> 3, tile = (warp >> 2) & 1;
+    const int slot = tid & (kTilePixels - 1);              // pixel of the CTA: tile * 128 + quadrant * 32 + lane
+    const int ptid = tid;                                  // 0..511 over both groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
-    const int64_t j = (int64_t)blockIdx.x * kProducerThreads + tid;
+    const int64_t j = (int64_t)blockIdx.x * kTilePixels + slot;
     const bool ok = j < n_pix;
-    const double rx = ok ? rprime[j] : 0.0, ry = ok ? rprime[pix_stride + j] : 0.0, rz = ok ? rprime[2 * pix_stride + j] : 0.0;
-    int n = 0;
-    for (int e = 0; e < n_collects; ++e) {
-      float* dcur = dsm + (size_t)(e & 1) * n_levels * NE;
-      for (int i = tid; i < n_levels * NE; i += kProducerThreads) {
-        const int l = i / NE, k = i - l * NE;
-        dcur[i] = weights[(size_t)e * weight_stride + (size_t)l * n_eig_pad + eig_offset + k];
-      }
-      for (int c = 0; c < n_chunks; ++c, ++n) {
+    PixelSplit q;
+    split_pixel(ok ? rprime[j] : 0.0, q.jx, q.lx, q.fx);
+    split_pixel(ok ? rprime[pix_stride + j] : 0.0, q.jy, q.ly, q.fy);
+    split_pixel(ok ? rprime[2 * pix_stride + j] : 0.0, q.jz, q.lz, q.fz);
+    float* mylev = lev + (size_t)group * n_levels * kTilePixels + slot;
+    int next_epi = 0;
+    for (int n = 0; n < total; ++n) {
+      if ((n & 1) == group) {
         const int sa = n % kSA, sb = n % kSB;
+        if (tid == 0) TR(0, 0);
         mbar_wait(&a_empty[sa], (uint32_t)(((n / kSA) & 1) ^ 1));
+        if (tid == 0) TR(0, 1);
         mbar_wait(&b_full[sb], (uint32_t)((n / kSB) & 1));
         tc_fence_after();
-        const double4* prow = reinterpret_cast<const double4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes);
-        const uint32_t a_col = tmem_base + lane_field + kColA + (uint32_t)(sa * 128 + tile * 64);
+        if (tid == 0) TR(0, 2);
+        const int4* rec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes);
+        const uint32_t a_col = tmem_base + lane_field + kColA + (uint32_t)sa * kColsStage + (uint32_t)tile * 2 * C::kColsHalf;
+        if (MODE == BB_TC_TF32) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {                      // 8 antennas -> 16 K-columns (cos, sin interleaved)
-          uint32_t hi[16], lo[16];
+          for (int h = 0; h < 2; ++h) {                    // 8 antennas -> 16 K-columns (cos, sin interleaved)
+            uint32_t hi[16], lo[16];
 #pragma unroll
-          for (int a = 0; a < 8; ++a) {
-            const double4 pp = prow[h * 8 + a];
-            float cs = 0.5f, sn = 0.25f;
-            if (!(dbg & 1)) phase_cs(pp.x, pp.y, pp.z, rx, ry, rz, cs, sn);
-            split_tf32(cs, hi[2 * a], lo[2 * a]);
-            split_tf32(sn, hi[2 * a + 1], lo[2 * a + 1]);
+            for (int a = 0; a < 8; ++a) {
+              const int4* r3 = rec + 3 * (h * 8 + a);
+              float cs, sn;
+              phase_cs(r3[0], *reinterpret_cast<const float4*>(r3 + 1), *reinterpret_cast<const float4*>(r3 + 2), q, cs, sn);
+              split_tf32(cs, hi[2 * a], lo[2 * a]);
+              split_tf32(sn, hi[2 * a + 1], lo[2 * a + 1]);
+            }
+            tmem_st16(a_col + h * 16, hi);
+            tmem_st16(a_col + C::kColsHalf + h * 16, lo);
           }
-          tmem_st16(a_col + h * 16, hi);
-          tmem_st16(a_col + 32 + h * 16, lo);
+        } else {
+          uint32_t hi[16], lo[16];                         // 16 antennas -> 16 packed (cos, sin) columns
+#pragma unroll
+          for (int a = 0; a < 16; ++a) {
+            const int4* r3 = rec + 3 * a;
+            float cs, sn;
+            phase_cs(r3[0], *reinterpret_cast<const float4*>(r3 + 1), *reinterpret_cast<const float4*>(r3 + 2), q, cs, sn);
+            split_f16(cs, sn, hi[a], lo[a]);
+          }
+          tmem_st16(a_col, hi);
+          tmem_st16(a_col + C::kColsHalf, lo);
         }
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&a_full[sa]);
+        if (tid == 0) TR(0, 3);
+        if (lane == 0) mbar_arrive(&a_full[2 * sa + tile]);
       }
-      // ---- a3: epilogue of this collect -------------------------------------------------------------
-      mbar_wait(d_full, (uint32_t)(e & 1));
-      tc_fence_after();
-      named_bar_sync(1, kProducerThreads);                 // weights of this collect are in shared memory
-      const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128);
-      float pw[kMaxNE];
+      // ---- a3: deferred epilogues (collect e once both groups had a go at collect e + 1) ---------------
+      while (next_epi < n_collects) {
+        const int e = next_epi;
+        const int due = min((e + 1) * n_chunks + 1, total - 1);
+        if (due > n) break;
+        ++next_epi;
+        const float* dcur = dsm + (size_t)(e & 1) * n_levels * NE;
+        mbar_wait(d_full, (uint32_t)(e & 1));
+        tc_fence_after();
+        named_bar_sync(1, kProducerWarps * 32);            // weights of collect e are in shared memory; buffer (e+1)&1 is free
+        float wnext[4];                                    // prefetch the weights of collect e + 1 (<= 2048 floats)
+        if (e + 1 < n_collects) {
 #pragma unroll
-      for (int g = 0; g < kMaxNE / 8; ++g) {
-        if (g * 8 < NE) {
-          float re[8], im[8];
-          tmem_ld8(d_col + g * 8, re);
-          tmem_ld8(d_col + NE + g * 8, im);
-          tmem_wait_ld();
+          for (int u = 0; u < 4; ++u) {
+            const int i = ptid + u * kProducerWarps * 32;
+            if (i < n_levels * NE) {
+              const int l = i / NE, k = i - l * NE;
+              wnext[u] = weights[(size_t)(e + 1) * weight_stride + (size_t)l * n_eig_pad + eig_offset + k];
+            }
+          }
+        }
+        const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128);
+        float pw[kMaxNE / 2];                              // this group's eigenpair octets: g = group, group + 2, ...
 #pragma unroll
-          for (int t = 0; t < 8; ++t) pw[g * 8 + t] = re[t] * re[t] + im[t] * im[t];
-        } else {
+        for (int gg = 0; gg < kMaxNE / 16; ++gg) {
+          const int g = 2 * gg + group;
+          if (g * 8 < NE) {
+            float re[8], im[8];
+            tmem_ld8(d_col + g * 8, re);
+            tmem_ld8(d_col + NE + g * 8, im);
+            tmem_wait_ld();
 #pragma unroll
-          for (int t = 0; t < 8; ++t) pw[g * 8 + t] = 0.f;
+            for (int t = 0; t < 8; ++t) pw[gg * 8 + t] = re[t] * re[t] + im[t] * im[t];
+          } else {
+#pragma unroll
+            for (int t = 0; t < 8; ++t) pw[gg * 8 + t] = 0.f;
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(d_empty);               // D may be overwritten by the next collect
+        for (int l = 0; l < n_levels; ++l) {
+          float sacc = 0.f;
+#pragma unroll
+          for (int gg = 0; gg < kMaxNE / 16; ++gg) {
+            const int g = 2 * gg + group;
+            if (g * 8 < NE) {
+              const float4* dl = reinterpret_cast<const float4*>(dcur + (size_t)l * NE + g * 8);
+              const float4 w0 = dl[0], w1 = dl[1];
+              sacc = fmaf(w0.x, pw[gg * 8], sacc);
+              sacc = fmaf(w0.y, pw[gg * 8 + 1], sacc);
+              sacc = fmaf(w0.z, pw[gg * 8 + 2], sacc);
+              sacc = fmaf(w0.w, pw[gg * 8 + 3], sacc);
+              sacc = fmaf(w1.x, pw[gg * 8 + 4], sacc);
+              sacc = fmaf(w1.y, pw[gg * 8 + 5], sacc);
+              sacc = fmaf(w1.z, pw[gg * 8 + 6], sacc);
+              sacc = fmaf(w1.w, pw[gg * 8 + 7], sacc);
+            }
+          }
+          mylev[(size_t)l * kTilePixels] += sacc;
+        }
+        if (e + 1 < n_collects) {
+          float* dnext = dsm + (size_t)((e + 1) & 1) * n_levels * NE;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = ptid + u * kProducerWarps * 32;
+            if (i < n_levels * NE) dnext[i] = wnext[u];
+          }
         }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(d_empty);                 // D may be overwritten by the next collect
-      for (int l = 0; l < n_levels; ++l) {
-        const float4* dl = reinterpret_cast<const float4*>(dcur + (size_t)l * NE);
-        float sacc = 0.f;
-#pragma unroll
-        for (int g = 0; g < kMaxNE / 4; ++g)
-          if (g * 4 < NE) {
-            const float4 w = dl[g];
-            sacc = fmaf(w.x, pw[4 * g], sacc);
-            sacc = fmaf(w.y, pw[4 * g + 1], sacc);
-            sacc = fmaf(w.z, pw[4 * g + 2], sacc);
-            sacc = fmaf(w.w, pw[4 * g + 3], sacc);
-          }
-        lev[(size_t)l * kProducerThreads + tid] += sacc;
-      }
     }
-    if (ok)
-      for (int l = 0; l < n_levels; ++l) img[(size_t)l * img_stride + j] += lev[(size_t)l * kProducerThreads + tid];
-  } else if (warp == 8) {
+    named_bar_sync(1, kProducerWarps * 32);                // both groups' level sums are complete
+    if (ok && group == 0)
+      for (int l = 0; l < n_levels; ++l)
+        img[(size_t)l * img_stride + j] += lev[(size_t)l * kTilePixels + slot] + lev[(size_t)(n_levels + l) * kTilePixels + slot];
+  } else if (warp == kProducerWarps) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
-      const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+      const uint32_t idesc = (1u << 4) | (C::kFmt << 7) | (C::kFmt << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+      const uint64_t desc0 = make_b_desc(smem_u32(stage_base), lbo, sbo);
+      const uint32_t step16 = (2 * lbo) >> 4;              // one MMA consumes two 16-byte core columns of B
       int n = 0;
       for (int e = 0; e < n_collects; ++e) {
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
           const int sa = n % kSA, sb = n % kSB;
-          mbar_wait(&a_full[sa], (uint32_t)((n / kSA) & 1));
+          TR(1, 0);
           mbar_wait(&b_full[sb], (uint32_t)((n / kSB) & 1));
-          tc_fence_after();
-          const uint32_t b_hi = smem_u32(stage_base + (size_t)sb * chunk_bytes), b_lo = b_hi + half_bytes;
+          const uint64_t b_hi = desc0 + (uint64_t)(((uint32_t)sb * chunk_bytes) >> 4);
+          const uint64_t b_lo = b_hi + (uint64_t)(half_bytes >> 4);
 #pragma unroll
           for (int t = 0; t < 2; ++t) {
+            mbar_wait(&a_full[2 * sa + t], (uint32_t)((n / kSA) & 1));
+            tc_fence_after();
+            if (t == 0) TR(1, 1); else TR(1, 2);
             const uint32_t d = tmem_base + kColD + t * 128;
-            const uint32_t a_hi = tmem_base + kColA + sa * 128 + t * 64, a_lo = a_hi + 32;
+            const uint32_t a_hi = tmem_base + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
 #pragma unroll
             for (int pass = 0; pass < 3; ++pass)
 #pragma unroll
-              for (int kk = 0; kk < kK / 8; ++kk) {
+              for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
                 const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
-                const uint64_t bd = make_b_desc((pass == 2 ? b_lo : b_hi) + kk * 2 * lbo, lbo, sbo);
-                if (!(dbg & 2)) mma_tf32_ts(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
+                const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
+                if (!(dbg & 2)) mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
               }
           }
           tc_commit(&a_empty[sa]);
-          if (CS > 1) tc_commit_mc(&b_empty[sb], (uint16_t)((1u << CS) - 1)); else tc_commit(&b_empty[sb]);
+          tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
+          TR(1, 3);
         }
       }
     }
   } else {
-    // ===================== B / p' loader =====================
+    // ===================== B / antenna-record loader =====================
     if (lane == 0) {
       for (int n = 0; n < total; ++n) {
         const int sb = n % kSB;
+        TR(2, 0);
         mbar_wait(&b_empty[sb], (uint32_t)(((n / kSB) & 1) ^ 1));
+        TR(2, 1);
         const int e = n / n_chunks, c = n - e * n_chunks;
         const unsigned char* src = packed + (size_t)e * packed_stride + slab_offset + (size_t)c * chunk_bytes;
         mbar_expect_tx(&b_full[sb], chunk_bytes);
-        if (CS > 1) {
-          const uint32_t part = chunk_bytes / CS, off = cluster_rank() * part;
-          bulk_g2s_mc(stage_base + (size_t)sb * chunk_bytes + off, src + off, part, &b_full[sb], (uint16_t)((1u << CS) - 1));
-        } else {
-          bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
-        }
+        bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
       }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (CS > 1) cluster_sync_all();          // no CTA exits while a peer may still multicast into it
-  if (warp == 8) {
+  if (warp == kProducerWarps) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols));
   }
 }
 
 // ---------------------------------------------------------------------------- preparation (a0'')
-// One thread per (antenna, eigenpair) of the padded operand: centre, fold the constant phase into B in fp64
-// (as prep_fp32_kernel), split hi/lo and scatter the four real entries into the UMMA canonical tiles.
+// One block per padded eigenpair column k: centre the antennas, fold the constant phase into B in fp64
+// (as prep_fp32_kernel), scale the column into FP16 range (FP16 mode), split hi/lo and scatter the four
+// real entries per antenna into the UMMA canonical tiles. The first column of a slab also writes the
+// antenna records of that slab's chunks.
+template <int MODE>
 __global__ void __launch_bounds__(256)
-prep_tc_kernel(PrepArgs a, int NE, int n_slabs, int n_chunks, int n_eig_pad, int n_ant_pad, size_t chunk_bytes) {
+prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, size_t chunk_bytes) {
+  using C = Cfg<MODE>;
   __shared__ double red[3][256];
+  __shared__ float redf[256];
   __shared__ double cen[3];
   const int tid = threadIdx.x;
+  const int k = blockIdx.x;
   double sx = 0, sy = 0, sz = 0;
+  float amax = 0.f;
   for (int i = tid; i < a.n_ant; i += 256) {
     sx += a.xyz[i]; sy += a.xyz[i + a.ldxyz]; sz += a.xyz[i + 2 * (size_t)a.ldxyz];
+    if (MODE == BB_TC_FP16 && k < a.n_eig) {
+      const bb_c32 b = a.B[i + (size_t)k * a.ldb];
+      amax = fmaxf(amax, fmaxf(fabsf(b.re), fabsf(b.im)));
+    }
   }
-  red[0][tid] = sx; red[1][tid] = sy; red[2][tid] = sz;
+  red[0][tid] = sx; red[1][tid] = sy; red[2][tid] = sz; redf[tid] = amax;
   __syncthreads();
   for (int w = 128; w > 0; w >>= 1) {
-    if (tid < w) { red[0][tid] += red[0][tid + w]; red[1][tid] += red[1][tid + w]; red[2][tid] += red[2][tid + w]; }
+    if (tid < w) {
+      red[0][tid] += red[0][tid + w]; red[1][tid] += red[1][tid + w]; red[2][tid] += red[2][tid + w];
+      redf[tid] = fmaxf(redf[tid], redf[tid + w]);
+    }
     __syncthreads();
   }
   if (tid < 3) cen[tid] = red[tid][0] / (double)a.n_ant;
   __syncthreads();
+  // FP16 mode: the column scale 2^ex puts the largest input component in [2^12, 2^13) (the phase fold can
+  // grow a component by sqrt 2; FP16 overflows at 65504); the weights absorb 2^(-2 ex) exactly.
+  int ex = 0;
+  if (MODE == BB_TC_FP16 && redf[0] > 0.f && isfinite(redf[0])) {
+    ex = 12 - ilogbf(redf[0]);
+    ex = ex > 40 ? 40 : (ex < -40 ? -40 : ex);
+  }
+  const double scale = ldexp(1.0, ex);
 
   const int N = 2 * NE;
-  const size_t half_bytes = (size_t)kK * N * 4;
-  const int64_t gid = (int64_t)blockIdx.x * 256 + tid;
-  const int64_t n_elem = (int64_t)n_ant_pad * n_eig_pad;
-  if (gid < n_elem) {
-    const int i = (int)(gid / n_eig_pad), k = (int)(gid - (int64_t)i * n_eig_pad);
+  const size_t half_bytes = (size_t)kK * N * C::kElem;
+  const int slab = k / NE, kk = k - slab * NE;
+  constexpr int kEpc = 16 / C::kElem;                      // elements per 16-byte core-matrix row
+  for (int i = tid; i < n_ant_pad; i += 256) {
     double px = 0, py = 0, pz = 0;
     float br = 0.f, bi = 0.f;
     if (i < a.n_ant) {
@@ -358,40 +494,93 @@ prep_tc_kernel(PrepArgs a, int NE, int n_slabs, int n_chunks, int n_eig_pad, int
         double sn, cs;
         sincospi(2.0 * th, &sn, &cs);
         const bb_c32 b = a.B[i + (size_t)k * a.ldb];
-        br = (float)((double)b.re * cs + (double)b.im * sn);
-        bi = (float)((double)b.im * cs - (double)b.re * sn);
+        br = (float)(((double)b.re * cs + (double)b.im * sn) * scale);
+        bi = (float)(((double)b.im * cs - (double)b.re * sn) * scale);
       }
     }
-    const int slab = k / NE, kk = k - slab * NE;
     const int c = i / kAC, ii = i - c * kAC;
     unsigned char* chunk = a.packed + ((size_t)slab * n_chunks + c) * chunk_bytes;
     auto put = [&](int n, int kidx, float v) {
-      const size_t off = (size_t)(kidx >> 2) * ((size_t)(N / 8) * 128) + (size_t)(n >> 3) * 128 + (size_t)(n & 7) * 16 + (size_t)(kidx & 3) * 4;
-      uint32_t hi, lo;
-      split_tf32(v, hi, lo);
-      *reinterpret_cast<uint32_t*>(chunk + off) = hi;
-      *reinterpret_cast<uint32_t*>(chunk + half_bytes + off) = lo;
+      const size_t off = (size_t)(kidx / kEpc) * ((size_t)(N / 8) * 128) + (size_t)(n >> 3) * 128 + (size_t)(n & 7) * 16 +
+                         (size_t)(kidx % kEpc) * C::kElem;
+      if (MODE == BB_TC_TF32) {
+        uint32_t hi, lo;
+        split_tf32(v, hi, lo);
+        *reinterpret_cast<uint32_t*>(chunk + off) = hi;
+        *reinterpret_cast<uint32_t*>(chunk + half_bytes + off) = lo;
+      } else {
+        const __half h = __float2half_rn(v);
+        *reinterpret_cast<__half*>(chunk + off) = h;
+        *reinterpret_cast<__half*>(chunk + half_bytes + off) = __float2half_rn(v - __half2float(h));
+      }
     };
     put(kk, 2 * ii, br);            // (Re,k)  x (i,cos)
     put(kk, 2 * ii + 1, bi);        // (Re,k)  x (i,sin)
     put(NE + kk, 2 * ii, bi);       // (Im',k) x (i,cos)
     put(NE + kk, 2 * ii + 1, -br);  // (Im',k) x (i,sin)
-    if (kk == 0) {
-      double* pp = reinterpret_cast<double*>(chunk + 2 * half_bytes) + (size_t)ii * 4;
-      pp[0] = px; pp[1] = py; pp[2] = pz; pp[3] = 0.0;
+    if (kk == 0) {                  // antenna record (zero for padding antennas)
+      const double tp = 6.283185307179586;
+      const double hx = rint(px * 256.0), hy = rint(py * 256.0), hz = rint(pz * 256.0);
+      int4 ih; float4 ph, pl;
+      ih.x = (int)hx; ih.y = (int)hy; ih.z = (int)hz; ih.w = 0;
+      ph.x = (float)(tp * hx / 256.0); ph.y = (float)(tp * hy / 256.0); ph.z = (float)(tp * hz / 256.0); ph.w = 0.f;
+      pl.x = (float)(tp * (px - hx / 256.0)); pl.y = (float)(tp * (py - hy / 256.0)); pl.z = (float)(tp * (pz - hz / 256.0)); pl.w = 0.f;
+      int4* rec = reinterpret_cast<int4*>(chunk + 2 * half_bytes + (size_t)ii * kRec);
+      rec[0] = ih;
+      rec[1] = *reinterpret_cast<int4*>(&ph);
+      rec[2] = *reinterpret_cast<int4*>(&pl);
     }
   }
-  const int64_t n_w = (int64_t)a.n_levels * n_eig_pad;
-  if (gid < n_w) {
-    const int l = (int)(gid / n_eig_pad), k = (int)(gid - (int64_t)l * n_eig_pad);
-    a.weights[gid] = (k < a.n_eig) ? a.D[l + (size_t)k * a.ldd] : 0.f;
+  // weights [level][n_eig_pad]; FP16 mode: |E|^2 comes out scaled by 2^(2 ex)
+  const float wscale = (float)ldexp(1.0, -2 * ex);
+  for (int l = tid; l < a.n_levels; l += 256)
+    a.weights[(size_t)l * n_eig_pad + k] = (k < a.n_eig) ? a.D[l + (size_t)k * a.ldd] * wscale : 0.f;
+}
+
+template <int MODE>
+int launch_prep(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
+  prep_tc_kernel<MODE><<<(unsigned)plan.n_eig_pad, 256, 0, st>>>(a, plan.eig_per_slab, plan.n_chunks, plan.n_eig_pad,
+                                                                 plan.n_ant_pad, plan.chunk_bytes);
+  BB_CUDA(cudaGetLastError());
+  return BB_OK;
+}
+
+template <int MODE>
+int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches, int dbg) {
+  using C = Cfg<MODE>;
+  const int NE = plan.eig_per_slab;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + 2 * (size_t)a.n_levels * kTilePixels * 4 +
+                      2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 2) * 8 + 16 + 1024;
+  auto kern = synth_tc_kernel<MODE>;
+  BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
+  for (int slab = 0; slab < plan.n_slabs; ++slab) {
+    kern<<<(unsigned)tiles, kThreadsTC, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
+                                                   (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights, a.weight_stride,
+                                                   plan.n_eig_pad, slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img,
+                                                   a.img_stride, dbg);
+    BB_CUDA(cudaGetLastError());
+    ++*launches;
   }
+#ifdef BB_TC_TRACE
+  if (getenv("BB_TC_TRACE")) {
+    cudaStreamSynchronize(st);
+    static long long h[4][128][4];
+    cudaMemcpyFromSymbol(h, g_trace, sizeof(h));
+    const long long t0 = h[0][0][0];
+    for (int n = 0; n < 128; ++n)
+      fprintf(stderr, "TR %3d P %6lld %6lld %6lld %6lld | M %6lld %6lld %6lld %6lld | L %6lld %6lld\n", n, h[0][n][0] - t0, h[0][n][1] - t0,
+              h[0][n][2] - t0, h[0][n][3] - t0, h[1][n][0] - t0, h[1][n][1] - t0, h[1][n][2] - t0, h[1][n][3] - t0, h[2][n][0] - t0, h[2][n][1] - t0);
+  }
+#endif
+  return BB_OK;
 }
 
 }  // namespace
 
-TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels) {
+TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels, int mode) {
   TcPlan p{};
+  p.mode = mode;
   p.AC = kAC;
   int ne = (n_eig + 7) / 8 * 8;
   if (ne > kMaxNE) ne = kMaxNE;
@@ -401,55 +590,21 @@ TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels) {
   p.n_chunks = (n_ant + kAC - 1) / kAC;
   p.n_eig_pad = p.n_slabs * ne;
   p.n_ant_pad = p.n_chunks * kAC;
-  p.chunk_bytes = 2 * (size_t)kK * p.NB * 4 + (size_t)kAC * 32;
+  const int elem = mode == BB_TC_FP16 ? 2 : 4;
+  p.chunk_bytes = 2 * (size_t)kK * p.NB * elem + (size_t)kAC * kRec;
   p.collect_bytes = (size_t)p.n_slabs * p.n_chunks * p.chunk_bytes;
   p.weight_floats = (size_t)n_levels * p.n_eig_pad;
   return p;
 }
 
 int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
-  const int64_t n_elem = (int64_t)plan.n_ant_pad * plan.n_eig_pad;
-  const int64_t n_w = (int64_t)a.n_levels * plan.n_eig_pad;
-  const int64_t n = n_elem > n_w ? n_elem : n_w;
-  prep_tc_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, plan.eig_per_slab, plan.n_slabs, plan.n_chunks,
-                                                              plan.n_eig_pad, plan.n_ant_pad, plan.chunk_bytes);
-  BB_CUDA(cudaGetLastError());
-  return BB_OK;
-}
-
-template <int CS>
-static int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches, int dbg) {
-  const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)kSB * plan.chunk_bytes, 1024) + (size_t)a.n_levels * kProducerThreads * 4 +
-                      2 * (size_t)a.n_levels * NE * 4 + (2 * kSB + 2 * kSA + 2) * 8 + 16 + 1024;
-  auto kern = synth_tc_kernel<CS>;
-  BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  int64_t tiles = (a.n_pix + kProducerThreads - 1) / kProducerThreads;
-  tiles = (tiles + CS - 1) / CS * CS;     // whole clusters; surplus CTAs own no pixel but take part in the B exchange
-  cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3((unsigned)tiles);
-  cfg.blockDim = dim3(kThreadsTC);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  for (int slab = 0; slab < plan.n_slabs; ++slab) {
-    BB_CUDA(cudaLaunchKernelEx(&cfg, kern, a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
-                               (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights, a.weight_stride, plan.n_eig_pad,
-                               slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img, a.img_stride, dbg));
-    ++*launches;
-  }
-  return BB_OK;
+  return plan.mode == BB_TC_FP16 ? launch_prep<BB_TC_FP16>(plan, a, st) : launch_prep<BB_TC_TF32>(plan, a, st);
 }
 
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
   *launches = 0;
   if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
-  const int dbg = getenv("BB_TC_DEBUG") ? atoi(getenv("BB_TC_DEBUG")) : 0;        // timing experiments only
-  const int cs = getenv("BB_TC_CLUSTER") ? atoi(getenv("BB_TC_CLUSTER")) : 2;
-  if (cs == 1) return launch_tc<1>(plan, a, st, launches, dbg);
-  if (cs == 4) return launch_tc<4>(plan, a, st, launches, dbg);
-  return launch_tc<2>(plan, a, st, launches, dbg);
+  // ablation knob for timing experiments only (results are wrong when set): 2 = no MMA
+  const int dbg = getenv("BB_TC_DEBUG") ? atoi(getenv("BB_TC_DEBUG")) : 0;
+  return plan.mode == BB_TC_FP16 ? launch_tc<BB_TC_FP16>(plan, a, st, launches, dbg) : launch_tc<BB_TC_TF32>(plan, a, st, launches, dbg);
 }

@@ -11,7 +11,7 @@ from helpers import assert_parity, eig_inputs, intervals_for, parity_numbers
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = ["fp32", "tf32x3"]
+VARIANTS = ["fp32", "tf32x3", "fp16x3"]
 
 
 @pytest.fixture(scope="module")
