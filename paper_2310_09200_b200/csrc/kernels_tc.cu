@@ -47,17 +47,26 @@ constexpr int kRec = 48;                // bytes of one antenna record {IH[3],0 
 constexpr int kMaxNE = 64;              // eigenpairs per slab
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t
-constexpr uint32_t kColA = 256;         // A stages
+constexpr int kLsTile = 512;            // bytes of one mini-GEMM B operand tile (16 antennas x 16 halves)
+constexpr int kApixTile = 4096;         // bytes of one mini-GEMM A operand tile (128 pixels x 16 halves)
 constexpr float kTwoPi = 6.283185307179586f;
 
 template <int MODE> struct Cfg;
-template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (tile, hi|lo)
+template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (tile, hi|lo); small phase part on CUDA cores
   static constexpr int kElem = 4, kSA = 2, kSB = 4, kColsHalf = kK, kMmaPerPass = kK / 8;
   static constexpr uint32_t kFmt = 2;   // instruction-descriptor operand format: TF32
+  static constexpr bool kLsOnTensor = false;
+  static constexpr uint32_t kColLs = 0;                  // unused
+  static constexpr uint32_t kColA = 256;                 // A stages start
+  static constexpr int kTail = kAC * kRec;               // chunk tail: antenna records
 };
 template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one antenna share a 32-bit column
-  static constexpr int kElem = 2, kSA = 4, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
+  static constexpr int kElem = 2, kSA = 3, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
   static constexpr uint32_t kFmt = 0;   // F16
+  static constexpr bool kLsOnTensor = true;              // small phase part as a K=16 mini-GEMM (see below)
+  static constexpr uint32_t kColLs = 256;                // ls buffers: kColLs + 32 buf + 16 tile, 16 columns each
+  static constexpr uint32_t kColA = 320;                 // A stages start
+  static constexpr int kTail = 2 * kLsTile + kAC * 16;   // chunk tail: B1 | B2 (mini-GEMM operands) | IH records
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -77,10 +86,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
       "@p bra DONE_%=;\n\t"
       "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity), "r"(0x989680u) : "memory");   // suspend-time hint: sleep, do not poll
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -91,6 +100,11 @@ __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence:
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool elect_one() {           // one lane of a converged warp
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
@@ -104,6 +118,12 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// D[tmem] (+)= A[smem desc] * B[smem desc]; kind::f16 (the mini-GEMM of the small phase part)
+__device__ __forceinline__ void mma_ss_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // shared-memory matrix descriptor: K-major, no swizzle; core matrix = 8 rows x 16 bytes, contiguous 128 B
 __device__ __forceinline__ uint64_t make_b_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
   uint64_t d = 0;
@@ -124,6 +144,14 @@ __device__ __forceinline__ void tmem_ld8(uint32_t addr, float (&v)[8]) {
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(addr));
 #pragma unroll
   for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t addr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(addr));
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
@@ -152,6 +180,14 @@ __device__ __forceinline__ void phase_cs(const int4& ih, const float4& ph, const
   // signed fraction of a turn, top 23 bits, as an exactly representable float (magic add, no I2F)
   const float f = __int_as_float(0x4B400000 + ((int)fr >> 9)) - 12582912.0f;
   const float x = fmaf(f, kTwoPi / 8388608.0f, ls);        // radians in (-pi - eps, pi + eps)
+  c = __cosf(x);
+  s = __sinf(x);
+}
+// Same with the small part ls (radians) taken from the mini-GEMM: one 16-byte word {IH_x, IH_y, IH_z, 0} per antenna.
+__device__ __forceinline__ void phase_cs_ls(const int4& ih, float ls, int jx, int jy, int jz, float& c, float& s) {
+  const uint32_t fr = (uint32_t)ih.x * (uint32_t)jx + (uint32_t)ih.y * (uint32_t)jy + (uint32_t)ih.z * (uint32_t)jz;
+  const float f = __int_as_float(0x4B400000 + ((int)fr >> 9)) - 12582912.0f;
+  const float x = fmaf(f, kTwoPi / 8388608.0f, ls);
   c = __cosf(x);
   s = __sinf(x);
 }
@@ -191,20 +227,21 @@ __global__ void __launch_bounds__(kThreadsTC, 1)
 synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                 const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                 const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset, int NE,
-                int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride, int dbg) {
+                int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride) {
   using C = Cfg<MODE>;
   constexpr int kSA = C::kSA, kSB = C::kSB;
+  constexpr uint32_t kColA = C::kColA;
   constexpr uint32_t kColsStage = 4 * C::kColsHalf;                 // 2 tiles x (hi | lo)
   static_assert(kColA + kSA * kColsStage <= kTmemCols, "TMEM budget");
-  static_assert(kSA % 2 == 0, "chunk parity must map to a fixed set of A stages");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int N = 2 * NE;
   const uint32_t half_bytes = (uint32_t)kK * N * C::kElem;          // one of B_hi / B_lo
-  const uint32_t chunk_bytes = 2 * half_bytes + kAC * kRec;
+  const uint32_t chunk_bytes = 2 * half_bytes + C::kTail;
   const uint32_t lbo = (uint32_t)(N / 8) * 128, sbo = 128;
 
   unsigned char* stage_base = smem_raw;
-  float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [2 groups][L][256]
+  unsigned char* apix = smem_raw + align_up((size_t)kSB * chunk_bytes, 1024);                    // [2 tiles][kApixTile]
+  float* lev = reinterpret_cast<float*>(apix + (C::kLsOnTensor ? 2 * kApixTile : 0));            // [2 groups][L][256]
   float* dsm = lev + 2 * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
   uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + 2 * (size_t)n_levels * NE);
   uint64_t* b_full = bars;                 // [kSB]
@@ -213,7 +250,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   uint64_t* a_empty = a_full + 2 * kSA;    // [kSA]
   uint64_t* d_full = a_empty + kSA;
   uint64_t* d_empty = d_full + 1;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
+  uint64_t* ls_full = d_empty + 1;         // [2 buffers]
+  uint64_t* ls_empty = ls_full + 2;        // [2 buffers]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ls_empty + 2);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
@@ -222,6 +261,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 1); }
     mbar_init(d_full, 1);
     mbar_init(d_empty, kProducerWarps);
+    for (int b = 0; b < 2; ++b) { mbar_init(&ls_full[b], 1); mbar_init(&ls_empty[b], kProducerWarps / 2); }
     fence_barrier_init();
   }
   if (warp == kProducerWarps) {
@@ -233,6 +273,31 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const int l = i / NE, k = i - l * NE;
     dsm[i] = weights[(size_t)l * n_eig_pad + eig_offset + k];
   }
+  // per-pixel constants of the phase generator (producer threads; both groups own the same 256 pixels)
+  const int slot = tid & (kTilePixels - 1);                // pixel of the CTA: tile * 128 + quadrant * 32 + lane
+  const int64_t j = (int64_t)blockIdx.x * kTilePixels + slot;
+  const bool ok = warp < kProducerWarps && j < n_pix;
+  PixelSplit q;
+  split_pixel(ok ? rprime[j] : 0.0, q.jx, q.lx, q.fx);
+  split_pixel(ok ? rprime[pix_stride + j] : 0.0, q.jy, q.ly, q.fy);
+  split_pixel(ok ? rprime[2 * pix_stride + j] : 0.0, q.jz, q.lz, q.fz);
+  if (C::kLsOnTensor && warp < kProducerWarps / 2) {
+    // A operand of the mini-GEMM, row = pixel, K = 16 halves (UMMA K-major, no swizzle; LBO 2048, SBO 128):
+    //   core column 0 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 0, 0}, core column 1 = lo of the same.
+    const float v[6] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz};
+    __align__(16) __half hi[8], lo[8];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {
+      const float x = t < 6 ? v[t] : 0.f;
+      hi[t] = __float2half_rn(x);
+      lo[t] = __float2half_rn(x - __half2float(hi[t]));
+    }
+    const int m = slot & 127;
+    unsigned char* row = apix + (size_t)(slot >> 7) * kApixTile + (size_t)(m >> 3) * 128 + (size_t)(m & 7) * 16;
+    *reinterpret_cast<int4*>(row) = *reinterpret_cast<const int4*>(hi);
+    *reinterpret_cast<int4*>(row + 2048) = *reinterpret_cast<const int4*>(lo);
+    fence_proxy_async_smem();                              // generic-proxy writes -> async-proxy (tensor core) reads
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -242,29 +307,23 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   if (warp < kProducerWarps) {
     // ===================== producers / epilogue: one pixel (TMEM lane) per thread =====================
     const int group = warp >> 3, tile = (warp >> 2) & 1;
-    const int slot = tid & (kTilePixels - 1);              // pixel of the CTA: tile * 128 + quadrant * 32 + lane
     const int ptid = tid;                                  // 0..511 over both groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
-    const int64_t j = (int64_t)blockIdx.x * kTilePixels + slot;
-    const bool ok = j < n_pix;
-    PixelSplit q;
-    split_pixel(ok ? rprime[j] : 0.0, q.jx, q.lx, q.fx);
-    split_pixel(ok ? rprime[pix_stride + j] : 0.0, q.jy, q.ly, q.fy);
-    split_pixel(ok ? rprime[2 * pix_stride + j] : 0.0, q.jz, q.lz, q.fz);
     float* mylev = lev + (size_t)group * n_levels * kTilePixels + slot;
     int next_epi = 0;
+    int sa = 0, sb = 0;
+    uint32_t pa = 0, pb = 0;                               // phase parities of the A / B stage rings
     for (int n = 0; n < total; ++n) {
       if ((n & 1) == group) {
-        const int sa = n % kSA, sb = n % kSB;
         if (tid == 0) TR(0, 0);
-        mbar_wait(&a_empty[sa], (uint32_t)(((n / kSA) & 1) ^ 1));
+        mbar_wait(&a_empty[sa], pa ^ 1);
         if (tid == 0) TR(0, 1);
-        mbar_wait(&b_full[sb], (uint32_t)((n / kSB) & 1));
+        mbar_wait(&b_full[sb], pb);
         tc_fence_after();
         if (tid == 0) TR(0, 2);
         const int4* rec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes);
         const uint32_t a_col = tmem_base + lane_field + kColA + (uint32_t)sa * kColsStage + (uint32_t)tile * 2 * C::kColsHalf;
-        if (MODE == BB_TC_TF32) {
+        if constexpr (MODE == BB_TC_TF32) {
 #pragma unroll
           for (int h = 0; h < 2; ++h) {                    // 8 antennas -> 16 K-columns (cos, sin interleaved)
             uint32_t hi[16], lo[16];
@@ -280,12 +339,21 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
             tmem_st16(a_col + C::kColsHalf + h * 16, lo);
           }
         } else {
+          // small phase part of this chunk from the mini-GEMM (radians), then release its TMEM buffer
+          float ls[16];
+          mbar_wait(&ls_full[group], (uint32_t)((n >> 1) & 1));
+          tc_fence_after();
+          tmem_ld16(tmem_base + lane_field + C::kColLs + (uint32_t)(group * 32 + tile * 16), ls);
+          tmem_wait_ld();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&ls_empty[group]);
+          const int4* ihrec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes + 2 * kLsTile);
           uint32_t hi[16], lo[16];                         // 16 antennas -> 16 packed (cos, sin) columns
 #pragma unroll
           for (int a = 0; a < 16; ++a) {
-            const int4* r3 = rec + 3 * a;
             float cs, sn;
-            phase_cs(r3[0], *reinterpret_cast<const float4*>(r3 + 1), *reinterpret_cast<const float4*>(r3 + 2), q, cs, sn);
+            phase_cs_ls(ihrec[a], ls[a], q.jx, q.jy, q.jz, cs, sn);
             split_f16(cs, sn, hi[a], lo[a]);
           }
           tmem_st16(a_col, hi);
@@ -297,6 +365,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         if (tid == 0) TR(0, 3);
         if (lane == 0) mbar_arrive(&a_full[2 * sa + tile]);
       }
+      if (++sa == kSA) { sa = 0; pa ^= 1; }
+      if (++sb == kSB) { sb = 0; pb ^= 1; }
       // ---- a3: deferred epilogues (collect e once both groups had a go at collect e + 1) ---------------
       while (next_epi < n_collects) {
         const int e = next_epi;
@@ -374,55 +444,92 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         img[(size_t)l * img_stride + j] += lev[(size_t)l * kTilePixels + slot] + lev[(size_t)(n_levels + l) * kTilePixels + slot];
   } else if (warp == kProducerWarps) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
+    // One elected thread; every operand is warp-uniform (the TMEM base is broadcast by shuffle and the
+    // thread is chosen by elect.sync) so that each tcgen05.mma costs a handful of uniform-datapath
+    // instructions: this single instruction stream paces the tensor pipe.
+    const uint32_t tb = __shfl_sync(0xffffffffu, tmem_base, 0);
+    if (elect_one()) {
       const uint32_t idesc = (1u << 4) | (C::kFmt << 7) | (C::kFmt << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
       const uint64_t desc0 = make_b_desc(smem_u32(stage_base), lbo, sbo);
       const uint32_t step16 = (2 * lbo) >> 4;              // one MMA consumes two 16-byte core columns of B
+      const uint32_t chunk16 = chunk_bytes >> 4, half16 = half_bytes >> 4;
       int n = 0;
+      int sa = 0, sb = 0;
+      uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
+      // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) for the 16 antennas of
+      // chunk m, two tiles, into TMEM buffer m & 1; issued two chunks ahead of the main MMAs of chunk m.
+      const uint32_t idesc_ls = (1u << 4) | ((uint32_t)(kAC >> 3) << 17) | ((128u >> 4) << 24);
+      const uint64_t desc_ls0 = make_b_desc(smem_u32(stage_base) + 2 * half_bytes, 2 * 128, 128);
+      const uint64_t desc_ap0 = make_b_desc(smem_u32(apix), 2048, 128);
+      int sbm = 0;
+      uint32_t pbm = 0;
+      auto issue_mini = [&](int m) {
+        mbar_wait(&b_full[sbm], pbm);
+        if (m >= 2) mbar_wait(&ls_empty[m & 1], (uint32_t)(((m >> 1) - 1) & 1));
+        tc_fence_after();
+        const uint64_t b1 = desc_ls0 + (uint64_t)((uint32_t)sbm * chunk16), b2 = b1 + (uint64_t)(kLsTile >> 4);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          const uint32_t d = tb + C::kColLs + (uint32_t)((m & 1) * 32 + t * 16);
+          const uint64_t ad = desc_ap0 + (uint64_t)((t * kApixTile) >> 4);
+          mma_ss_f16(d, ad, b1, idesc_ls, 0u);             // A_hi B_hi + A_lo B_hi
+          mma_ss_f16(d, ad, b2, idesc_ls, 1u);             // A_hi B_lo
+        }
+        tc_commit(&ls_full[m & 1]);
+        if (++sbm == kSB) { sbm = 0; pbm ^= 1; }
+      };
+      if (C::kLsOnTensor) {
+        if (total > 0) issue_mini(0);
+        if (total > 1) issue_mini(1);
+      }
       for (int e = 0; e < n_collects; ++e) {
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
-          const int sa = n % kSA, sb = n % kSB;
           TR(1, 0);
-          mbar_wait(&b_full[sb], (uint32_t)((n / kSB) & 1));
-          const uint64_t b_hi = desc0 + (uint64_t)(((uint32_t)sb * chunk_bytes) >> 4);
-          const uint64_t b_lo = b_hi + (uint64_t)(half_bytes >> 4);
+          if (C::kLsOnTensor && n + 2 < total) issue_mini(n + 2);
+          mbar_wait(&b_full[sb], pb);
+          const uint64_t b_hi = desc0 + (uint64_t)((uint32_t)sb * chunk16);
+          const uint64_t b_lo = b_hi + (uint64_t)half16;
 #pragma unroll
           for (int t = 0; t < 2; ++t) {
-            mbar_wait(&a_full[2 * sa + t], (uint32_t)((n / kSA) & 1));
+            mbar_wait(&a_full[2 * sa + t], pa);
             tc_fence_after();
             if (t == 0) TR(1, 1); else TR(1, 2);
-            const uint32_t d = tmem_base + kColD + t * 128;
-            const uint32_t a_hi = tmem_base + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
+            const uint32_t d = tb + kColD + t * 128;
+            const uint32_t a_hi = tb + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
 #pragma unroll
             for (int pass = 0; pass < 3; ++pass)
 #pragma unroll
               for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
                 const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
                 const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
-                if (!(dbg & 2)) mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
+                mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
               }
           }
           tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
           TR(1, 3);
+          if (++sa == kSA) { sa = 0; pa ^= 1; }
+          if (++sb == kSB) { sb = 0; pb ^= 1; }
         }
       }
     }
   } else {
     // ===================== B / antenna-record loader =====================
-    if (lane == 0) {
+    if (elect_one()) {
+      int sb = 0, e = 0, c = 0;
+      uint32_t pb = 1;
       for (int n = 0; n < total; ++n) {
-        const int sb = n % kSB;
         TR(2, 0);
-        mbar_wait(&b_empty[sb], (uint32_t)(((n / kSB) & 1) ^ 1));
+        mbar_wait(&b_empty[sb], pb);
         TR(2, 1);
-        const int e = n / n_chunks, c = n - e * n_chunks;
         const unsigned char* src = packed + (size_t)e * packed_stride + slab_offset + (size_t)c * chunk_bytes;
         mbar_expect_tx(&b_full[sb], chunk_bytes);
         bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
+        if (++sb == kSB) { sb = 0; pb ^= 1; }
+        if (++c == n_chunks) { c = 0; ++e; }
       }
     }
   }
@@ -518,17 +625,40 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
     put(kk, 2 * ii + 1, bi);        // (Re,k)  x (i,sin)
     put(NE + kk, 2 * ii, bi);       // (Im',k) x (i,cos)
     put(NE + kk, 2 * ii + 1, -br);  // (Im',k) x (i,sin)
-    if (kk == 0) {                  // antenna record (zero for padding antennas)
+    if (kk == 0) {                  // per-antenna phase-generator data (zero for padding antennas)
       const double tp = 6.283185307179586;
       const double hx = rint(px * 256.0), hy = rint(py * 256.0), hz = rint(pz * 256.0);
-      int4 ih; float4 ph, pl;
+      int4 ih;
       ih.x = (int)hx; ih.y = (int)hy; ih.z = (int)hz; ih.w = 0;
-      ph.x = (float)(tp * hx / 256.0); ph.y = (float)(tp * hy / 256.0); ph.z = (float)(tp * hz / 256.0); ph.w = 0.f;
-      pl.x = (float)(tp * (px - hx / 256.0)); pl.y = (float)(tp * (py - hy / 256.0)); pl.z = (float)(tp * (pz - hz / 256.0)); pl.w = 0.f;
-      int4* rec = reinterpret_cast<int4*>(chunk + 2 * half_bytes + (size_t)ii * kRec);
-      rec[0] = ih;
-      rec[1] = *reinterpret_cast<int4*>(&ph);
-      rec[2] = *reinterpret_cast<int4*>(&pl);
+      unsigned char* tail = chunk + 2 * half_bytes;
+      if (MODE == BB_TC_TF32) {
+        float4 ph, pl;
+        ph.x = (float)(tp * hx / 256.0); ph.y = (float)(tp * hy / 256.0); ph.z = (float)(tp * hz / 256.0); ph.w = 0.f;
+        pl.x = (float)(tp * (px - hx / 256.0)); pl.y = (float)(tp * (py - hy / 256.0)); pl.z = (float)(tp * (pz - hz / 256.0)); pl.w = 0.f;
+        int4* rec = reinterpret_cast<int4*>(tail + (size_t)ii * kRec);
+        rec[0] = ih;
+        rec[1] = *reinterpret_cast<int4*>(&ph);
+        rec[2] = *reinterpret_cast<int4*>(&pl);
+      } else {
+        // mini-GEMM B operand rows (N = 16 antennas, K = 16 halves, UMMA K-major no swizzle, LBO 256, SBO 128):
+        //   v = {2 pi PH 2^-24 (x,y,z), 2 pi PL (x,y,z), 0, 0};  B1 = [hi(v) | hi(v)],  B2 = [lo(v) | 0]
+        const double v[6] = {tp * hx / 256.0 / 16777216.0, tp * hy / 256.0 / 16777216.0, tp * hz / 256.0 / 16777216.0,
+                             tp * (px - hx / 256.0), tp * (py - hy / 256.0), tp * (pz - hz / 256.0)};
+        __align__(16) __half hi[8], lo[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          const float x = t < 6 ? (float)v[t] : 0.f;
+          hi[t] = __float2half_rn(x);
+          lo[t] = __float2half_rn(x - __half2float(hi[t]));
+        }
+        unsigned char* row = tail + (size_t)(ii >> 3) * 128 + (size_t)(ii & 7) * 16;
+        const int4 z = make_int4(0, 0, 0, 0);
+        *reinterpret_cast<int4*>(row) = *reinterpret_cast<const int4*>(hi);                    // B1 core column 0
+        *reinterpret_cast<int4*>(row + 256) = *reinterpret_cast<const int4*>(hi);              // B1 core column 1
+        *reinterpret_cast<int4*>(row + kLsTile) = *reinterpret_cast<const int4*>(lo);          // B2 core column 0
+        *reinterpret_cast<int4*>(row + kLsTile + 256) = z;                                     // B2 core column 1
+        reinterpret_cast<int4*>(tail + 2 * kLsTile)[ii] = ih;
+      }
     }
   }
   // weights [level][n_eig_pad]; FP16 mode: |E|^2 comes out scaled by 2^(2 ex)
@@ -546,11 +676,11 @@ int launch_prep(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
 }
 
 template <int MODE>
-int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches, int dbg) {
+int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + 2 * (size_t)a.n_levels * kTilePixels * 4 +
-                      2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 2) * 8 + 16 + 1024;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + (C::kLsOnTensor ? 2 * kApixTile : 0) +
+                      2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 6) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
@@ -558,7 +688,7 @@ int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* laun
     kern<<<(unsigned)tiles, kThreadsTC, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
                                                    (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights, a.weight_stride,
                                                    plan.n_eig_pad, slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img,
-                                                   a.img_stride, dbg);
+                                                   a.img_stride);
     BB_CUDA(cudaGetLastError());
     ++*launches;
   }
@@ -591,7 +721,7 @@ TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels, int mode) {
   p.n_eig_pad = p.n_slabs * ne;
   p.n_ant_pad = p.n_chunks * kAC;
   const int elem = mode == BB_TC_FP16 ? 2 : 4;
-  p.chunk_bytes = 2 * (size_t)kK * p.NB * elem + (size_t)kAC * kRec;
+  p.chunk_bytes = 2 * (size_t)kK * p.NB * elem + (size_t)(mode == BB_TC_FP16 ? Cfg<BB_TC_FP16>::kTail : Cfg<BB_TC_TF32>::kTail);
   p.collect_bytes = (size_t)p.n_slabs * p.n_chunks * p.chunk_bytes;
   p.weight_floats = (size_t)n_levels * p.n_eig_pad;
   return p;
@@ -604,7 +734,5 @@ int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
   *launches = 0;
   if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
-  // ablation knob for timing experiments only (results are wrong when set): 2 = no MMA
-  const int dbg = getenv("BB_TC_DEBUG") ? atoi(getenv("BB_TC_DEBUG")) : 0;
-  return plan.mode == BB_TC_FP16 ? launch_tc<BB_TC_FP16>(plan, a, st, launches, dbg) : launch_tc<BB_TC_TF32>(plan, a, st, launches, dbg);
+  return plan.mode == BB_TC_FP16 ? launch_tc<BB_TC_FP16>(plan, a, st, launches) : launch_tc<BB_TC_TF32>(plan, a, st, launches);
 }
