@@ -23,13 +23,13 @@
 //   three wrapping 32-bit IMADs give the large part exactly; the small part (< 2^-6 turns) is 6 fp32 FMAs.
 //   The 32-bit fraction is converted with the 1.5*2^23 magic-add (no I2F on the MUFU pipe), then MUFU.SIN/COS.
 //
-// CTA = 2 pixel tiles of 128 (256 pixels), 576 threads, 1 CTA per SM, all 512 TMEM columns:
+// CTA = 2 pixel tiles of 128 (256 pixels), 608 threads, 1 CTA per SM, all 512 TMEM columns:
 //   warps 0-15 producers + epilogue (two groups alternating chunks): phase generator, hi/lo split,
 //              tcgen05.st of their A rows straight into TMEM (A operand from TMEM: no smem round trip);
 //              per collect: tcgen05.ld of D, |E|^2, level weights, level sums.
-//   warp 16    one elected thread issues tcgen05.mma.cta_group::1 (A from TMEM, B from smem descriptors)
-//              and tcgen05.commit to the stage / accumulator mbarriers; owns TMEM alloc.
-//   warp 17    one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
+//   warps 16,17 one elected thread per pixel tile issues tcgen05.mma.cta_group::1 (A from TMEM, B from smem
+//              descriptors) and tcgen05.commit to the stage / accumulator mbarriers; warp 16 owns TMEM alloc.
+//   warp 18    one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
 //              layout, written by prep_tc_kernel) global -> shared with cp.async.bulk on mbarriers.
 #include "internal.h"
 #include <cuda_fp16.h>
@@ -40,7 +40,7 @@ namespace {
 
 constexpr int kTilePixels = 256;        // pixels per CTA (2 tiles of 128 TMEM lanes)
 constexpr int kProducerWarps = 16;      // 2 groups x 2 tiles x 4 lane quadrants
-constexpr int kThreadsTC = (kProducerWarps + 2) * 32;
+constexpr int kThreadsTC = (kProducerWarps + 3) * 32;   // + one MMA issuer per tile + the loader
 constexpr int kAC = 16;                 // antennas per chunk
 constexpr int kK = 2 * kAC;             // K-columns (cos, sin per antenna) per chunk and pass
 constexpr int kRec = 48;                // bytes of one antenna record {IH[3],0 | 2pi PH[3],0 | 2pi PL[3],0}
@@ -90,6 +90,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "@p bra DONE_%=;\n\t"
       "bra WAIT_%=;\n\t"
       "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity), "r"(0x989680u) : "memory");   // suspend-time hint: sleep, do not poll
+}
+// Wait for two barriers at once: both try_waits are in flight together, so the common "both already complete"
+// case costs one barrier latency. Safe only when neither barrier can complete a further phase before this
+// thread acts (true for every pair used below).
+__device__ __forceinline__ void mbar_wait2(uint64_t* bar_a, uint32_t parity_a, uint64_t* bar_b, uint32_t parity_b) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %4;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 q, [%2], %3, %4;\n\t"
+      "and.pred p, p, q;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar_a)), "r"(parity_a), "r"(smem_u32(bar_b)), "r"(parity_b), "r"(0x989680u) : "memory");
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -183,11 +197,13 @@ __device__ __forceinline__ void phase_cs(const int4& ih, const float4& ph, const
   c = __cosf(x);
   s = __sinf(x);
 }
-// Same with the small part ls (radians) taken from the mini-GEMM: one 16-byte word {IH_x, IH_y, IH_z, 0} per antenna.
-__device__ __forceinline__ void phase_cs_ls(const int4& ih, float ls, int jx, int jy, int jz, float& c, float& s) {
+// Same with the small part taken from the mini-GEMM, which also carries the constant -2 pi: lsm = ls - 2 pi.
+// One 16-byte word {IH_x, IH_y, IH_z, 0} per antenna. F = 1 + frac in [1, 2) is built by an integer add on the
+// exponent pattern of 1.0f, so x = 2 pi F + lsm = 2 pi frac + ls lies in [0, 2 pi): 3 IMAD, LEA.HI, FFMA, then MUFU.
+__device__ __forceinline__ void phase_cs_ls(const int4& ih, float lsm, int jx, int jy, int jz, float& c, float& s) {
   const uint32_t fr = (uint32_t)ih.x * (uint32_t)jx + (uint32_t)ih.y * (uint32_t)jy + (uint32_t)ih.z * (uint32_t)jz;
-  const float f = __int_as_float(0x4B400000 + ((int)fr >> 9)) - 12582912.0f;
-  const float x = fmaf(f, kTwoPi / 8388608.0f, ls);
+  const float F = __uint_as_float(0x3F800000u + (fr >> 9));
+  const float x = fmaf(F, kTwoPi, lsm);
   c = __cosf(x);
   s = __sinf(x);
 }
@@ -195,12 +211,15 @@ __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) 
   hi = __float_as_uint(x) & 0xFFFFE000u;
   lo = __float_as_uint(x - __uint_as_float(hi));
 }
-// (cos, sin) -> packed FP16 pairs: hi = rn16(x), lo = rn16(x - hi); K order (cos, sin) = (low, high) half
+// (cos, sin) -> packed FP16 pairs: hi = rn16(x), lo = rn16(x - hi); K order (cos, sin) = (low, high) half.
+// x - hi is one mixed-precision FMA per value (fma.rn.f32.f16: hi * -1 + x, SASS FHFMA).
 __device__ __forceinline__ void split_f16(float c, float s, uint32_t& hi, uint32_t& lo) {
   const __half2 h = __floats2half2_rn(c, s);
-  const float2 hf = __half22float2(h);
-  const __half2 l = __floats2half2_rn(c - hf.x, s - hf.y);
   hi = *reinterpret_cast<const uint32_t*>(&h);
+  float lc, lsn;
+  asm("{\n\t.reg .f16 a, b, m;\n\tmov.b32 {a, b}, %2;\n\tmov.b16 m, 0xBC00;\n\t"
+      "fma.rn.f32.f16 %0, a, m, %3;\n\tfma.rn.f32.f16 %1, b, m, %4;\n\t}" : "=f"(lc), "=f"(lsn) : "r"(hi), "f"(c), "f"(s));
+  const __half2 l = __floats2half2_rn(lc, lsn);
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
@@ -250,18 +269,18 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   uint64_t* a_empty = a_full + 2 * kSA;    // [kSA]
   uint64_t* d_full = a_empty + kSA;
   uint64_t* d_empty = d_full + 1;
-  uint64_t* ls_full = d_empty + 1;         // [2 buffers]
-  uint64_t* ls_empty = ls_full + 2;        // [2 buffers]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ls_empty + 2);
+  uint64_t* ls_full = d_empty + 1;         // [2 buffers][2 tiles]
+  uint64_t* ls_empty = ls_full + 4;        // [2 buffers][2 tiles]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ls_empty + 4);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   if (tid == 0) {
-    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 1); }
-    for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 1); }
-    mbar_init(d_full, 1);
+    for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 2); }      // 2: one commit per tile issuer
+    for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 2); }
+    mbar_init(d_full, 2);
     mbar_init(d_empty, kProducerWarps);
-    for (int b = 0; b < 2; ++b) { mbar_init(&ls_full[b], 1); mbar_init(&ls_empty[b], kProducerWarps / 2); }
+    for (int b = 0; b < 4; ++b) { mbar_init(&ls_full[b], 1); mbar_init(&ls_empty[b], 4); }
     fence_barrier_init();
   }
   if (warp == kProducerWarps) {
@@ -283,12 +302,12 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   split_pixel(ok ? rprime[2 * pix_stride + j] : 0.0, q.jz, q.lz, q.fz);
   if (C::kLsOnTensor && warp < kProducerWarps / 2) {
     // A operand of the mini-GEMM, row = pixel, K = 16 halves (UMMA K-major, no swizzle; LBO 2048, SBO 128):
-    //   core column 0 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 0, 0}, core column 1 = lo of the same.
-    const float v[6] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz};
+    //   core column 0 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 1, 0}, core column 1 = lo of the same.
+    const float v[7] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz, 1.0f};
     __align__(16) __half hi[8], lo[8];
 #pragma unroll
     for (int t = 0; t < 8; ++t) {
-      const float x = t < 6 ? v[t] : 0.f;
+      const float x = t < 7 ? v[t] : 0.f;
       hi[t] = __float2half_rn(x);
       lo[t] = __float2half_rn(x - __half2float(hi[t]));
     }
@@ -310,11 +329,12 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const int ptid = tid;                                  // 0..511 over both groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
     float* mylev = lev + (size_t)group * n_levels * kTilePixels + slot;
-    int next_epi = 0;
-    int sa = 0, sb = 0;
+    int next_epi = 0, next_due = n_chunks;                 // epilogue e is due once this group produced a chunk of collect e + 1
+    int sa = group, sb = group;                            // this group's chunks: n = group, group + 2, ...
     uint32_t pa = 0, pb = 0;                               // phase parities of the A / B stage rings
-    for (int n = 0; n < total; ++n) {
-      if ((n & 1) == group) {
+    for (int n = group;; n += 2) {
+      const bool have = n < total;
+      if (have) {
         if (tid == 0) TR(0, 0);
         mbar_wait(&a_empty[sa], pa ^ 1);
         if (tid == 0) TR(0, 1);
@@ -339,15 +359,15 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
             tmem_st16(a_col + C::kColsHalf + h * 16, lo);
           }
         } else {
-          // small phase part of this chunk from the mini-GEMM (radians), then release its TMEM buffer
+          // small phase part of this chunk (minus 2 pi) from the mini-GEMM, then release its TMEM buffer
           float ls[16];
-          mbar_wait(&ls_full[group], (uint32_t)((n >> 1) & 1));
+          mbar_wait(&ls_full[2 * group + tile], (uint32_t)((n >> 1) & 1));
           tc_fence_after();
           tmem_ld16(tmem_base + lane_field + C::kColLs + (uint32_t)(group * 32 + tile * 16), ls);
           tmem_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(&ls_empty[group]);
+          if (lane == 0) mbar_arrive(&ls_empty[2 * group + tile]);
           const int4* ihrec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes + 2 * kLsTile);
           uint32_t hi[16], lo[16];                         // 16 antennas -> 16 packed (cos, sin) columns
 #pragma unroll
@@ -365,14 +385,13 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         if (tid == 0) TR(0, 3);
         if (lane == 0) mbar_arrive(&a_full[2 * sa + tile]);
       }
-      if (++sa == kSA) { sa = 0; pa ^= 1; }
-      if (++sb == kSB) { sb = 0; pb ^= 1; }
-      // ---- a3: deferred epilogues (collect e once both groups had a go at collect e + 1) ---------------
-      while (next_epi < n_collects) {
+      sa += 2; if (sa >= kSA) { sa -= kSA; pa ^= 1; }
+      sb += 2; if (sb >= kSB) { sb -= kSB; pb ^= 1; }
+      // ---- a3: deferred epilogues (collect e once this group had a go at collect e + 1, or at the end) ----
+      while (next_epi < n_collects && (next_due <= n || !have)) {
         const int e = next_epi;
-        const int due = min((e + 1) * n_chunks + 1, total - 1);
-        if (due > n) break;
         ++next_epi;
+        next_due += n_chunks;
         const float* dcur = dsm + (size_t)(e & 1) * n_levels * NE;
         mbar_wait(d_full, (uint32_t)(e & 1));
         tc_fence_after();
@@ -437,45 +456,45 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           }
         }
       }
+      if (!have) break;
     }
     named_bar_sync(1, kProducerWarps * 32);                // both groups' level sums are complete
     if (ok && group == 0)
       for (int l = 0; l < n_levels; ++l)
         img[(size_t)l * img_stride + j] += lev[(size_t)l * kTilePixels + slot] + lev[(size_t)(n_levels + l) * kTilePixels + slot];
-  } else if (warp == kProducerWarps) {
-    // ===================== MMA issuer =====================
-    // One elected thread; every operand is warp-uniform (the TMEM base is broadcast by shuffle and the
+  } else if (warp < kProducerWarps + 2) {
+    // ===================== MMA issuers: one warp per pixel tile =====================
+    // One elected thread each; every operand is warp-uniform (the TMEM base is broadcast by shuffle and the
     // thread is chosen by elect.sync) so that each tcgen05.mma costs a handful of uniform-datapath
-    // instructions: this single instruction stream paces the tensor pipe.
+    // instructions. A blocking mbarrier wait costs ~90 cycles even when already complete and the issuer is a
+    // single serial instruction stream, so the two tiles get independent issuers and waits are paired.
+    const int t = warp - kProducerWarps;                   // tile of this issuer
     const uint32_t tb = __shfl_sync(0xffffffffu, tmem_base, 0);
     if (elect_one()) {
       const uint32_t idesc = (1u << 4) | (C::kFmt << 7) | (C::kFmt << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
       const uint64_t desc0 = make_b_desc(smem_u32(stage_base), lbo, sbo);
       const uint32_t step16 = (2 * lbo) >> 4;              // one MMA consumes two 16-byte core columns of B
       const uint32_t chunk16 = chunk_bytes >> 4, half16 = half_bytes >> 4;
+      const uint32_t d = tb + kColD + t * 128;
       int n = 0;
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
-      // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) for the 16 antennas of
-      // chunk m, two tiles, into TMEM buffer m & 1; issued two chunks ahead of the main MMAs of chunk m.
+      // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) - 2 pi for the 16
+      // antennas of chunk m into TMEM buffer m & 1; issued two chunks ahead of the main MMAs of chunk m.
       const uint32_t idesc_ls = (1u << 4) | ((uint32_t)(kAC >> 3) << 17) | ((128u >> 4) << 24);
       const uint64_t desc_ls0 = make_b_desc(smem_u32(stage_base) + 2 * half_bytes, 2 * 128, 128);
-      const uint64_t desc_ap0 = make_b_desc(smem_u32(apix), 2048, 128);
+      const uint64_t desc_ap = make_b_desc(smem_u32(apix) + t * kApixTile, 2048, 128);
       int sbm = 0;
       uint32_t pbm = 0;
       auto issue_mini = [&](int m) {
-        mbar_wait(&b_full[sbm], pbm);
-        if (m >= 2) mbar_wait(&ls_empty[m & 1], (uint32_t)(((m >> 1) - 1) & 1));
+        if (m >= 2) mbar_wait2(&b_full[sbm], pbm, &ls_empty[2 * (m & 1) + t], (uint32_t)(((m >> 1) - 1) & 1));
+        else mbar_wait(&b_full[sbm], pbm);
         tc_fence_after();
         const uint64_t b1 = desc_ls0 + (uint64_t)((uint32_t)sbm * chunk16), b2 = b1 + (uint64_t)(kLsTile >> 4);
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-          const uint32_t d = tb + C::kColLs + (uint32_t)((m & 1) * 32 + t * 16);
-          const uint64_t ad = desc_ap0 + (uint64_t)((t * kApixTile) >> 4);
-          mma_ss_f16(d, ad, b1, idesc_ls, 0u);             // A_hi B_hi + A_lo B_hi
-          mma_ss_f16(d, ad, b2, idesc_ls, 1u);             // A_hi B_lo
-        }
-        tc_commit(&ls_full[m & 1]);
+        const uint32_t dl = tb + C::kColLs + (uint32_t)((m & 1) * 32 + t * 16);
+        mma_ss_f16(dl, desc_ap, b1, idesc_ls, 0u);         // A_hi B_hi + A_lo B_hi
+        mma_ss_f16(dl, desc_ap, b2, idesc_ls, 1u);         // A_hi B_lo
+        tc_commit(&ls_full[2 * (m & 1) + t]);
         if (++sbm == kSB) { sbm = 0; pbm ^= 1; }
       };
       if (C::kLsOnTensor) {
@@ -486,31 +505,31 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
-          TR(1, 0);
-          if (C::kLsOnTensor && n + 2 < total) issue_mini(n + 2);
-          mbar_wait(&b_full[sb], pb);
+          if (t == 0) TR(1, 0);
+          if (C::kLsOnTensor) {
+            if (n + 2 < total) issue_mini(n + 2);          // (its b_full wait covered chunk n two iterations ago)
+            if (t == 0) TR(1, 1);
+            mbar_wait(&a_full[2 * sa + t], pa);
+          } else {
+            mbar_wait2(&b_full[sb], pb, &a_full[2 * sa + t], pa);
+          }
+          tc_fence_after();
+          if (t == 0) TR(1, 2);
           const uint64_t b_hi = desc0 + (uint64_t)((uint32_t)sb * chunk16);
           const uint64_t b_lo = b_hi + (uint64_t)half16;
+          const uint32_t a_hi = tb + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
 #pragma unroll
-          for (int t = 0; t < 2; ++t) {
-            mbar_wait(&a_full[2 * sa + t], pa);
-            tc_fence_after();
-            if (t == 0) TR(1, 1); else TR(1, 2);
-            const uint32_t d = tb + kColD + t * 128;
-            const uint32_t a_hi = tb + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
+          for (int pass = 0; pass < 3; ++pass)
 #pragma unroll
-            for (int pass = 0; pass < 3; ++pass)
-#pragma unroll
-              for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
-                const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
-                const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
-                mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
-              }
-          }
+            for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
+              const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
+              const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
+              mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
+            }
           tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
-          TR(1, 3);
+          if (t == 0) TR(1, 3);
           if (++sa == kSA) { sa = 0; pa ^= 1; }
           if (++sb == kSB) { sb = 0; pb ^= 1; }
         }
@@ -641,13 +660,13 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
         rec[2] = *reinterpret_cast<int4*>(&pl);
       } else {
         // mini-GEMM B operand rows (N = 16 antennas, K = 16 halves, UMMA K-major no swizzle, LBO 256, SBO 128):
-        //   v = {2 pi PH 2^-24 (x,y,z), 2 pi PL (x,y,z), 0, 0};  B1 = [hi(v) | hi(v)],  B2 = [lo(v) | 0]
-        const double v[6] = {tp * hx / 256.0 / 16777216.0, tp * hy / 256.0 / 16777216.0, tp * hz / 256.0 / 16777216.0,
-                             tp * (px - hx / 256.0), tp * (py - hy / 256.0), tp * (pz - hz / 256.0)};
+        //   v = {2 pi PH 2^-24 (x,y,z), 2 pi PL (x,y,z), -2 pi, 0};  B1 = [hi(v) | hi(v)],  B2 = [lo(v) | 0]
+        const double v[7] = {tp * hx / 256.0 / 16777216.0, tp * hy / 256.0 / 16777216.0, tp * hz / 256.0 / 16777216.0,
+                             tp * (px - hx / 256.0), tp * (py - hy / 256.0), tp * (pz - hz / 256.0), -tp};
         __align__(16) __half hi[8], lo[8];
 #pragma unroll
         for (int t = 0; t < 8; ++t) {
-          const float x = t < 6 ? (float)v[t] : 0.f;
+          const float x = t < 7 ? (float)v[t] : 0.f;
           hi[t] = __float2half_rn(x);
           lo[t] = __float2half_rn(x - __half2float(hi[t]));
         }
@@ -680,7 +699,7 @@ int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* laun
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
   const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + (C::kLsOnTensor ? 2 * kApixTile : 0) +
-                      2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 6) * 8 + 16 + 1024;
+                      2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 10) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
