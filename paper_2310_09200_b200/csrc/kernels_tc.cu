@@ -48,7 +48,6 @@ constexpr int kMaxNE = 64;              // eigenpairs per slab
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t
 constexpr int kLsTile = 512;            // bytes of one mini-GEMM B operand tile (16 antennas x 16 halves)
-constexpr int kApixTile = 4096;         // bytes of one mini-GEMM A operand tile (128 pixels x 16 halves)
 constexpr float kTwoPi = 6.283185307179586f;
 
 template <int MODE> struct Cfg;
@@ -64,8 +63,8 @@ template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one an
   static constexpr int kElem = 2, kSA = 3, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
   static constexpr uint32_t kFmt = 0;   // F16
   static constexpr bool kLsOnTensor = true;              // small phase part as a K=16 mini-GEMM (see below)
-  static constexpr uint32_t kColLs = 256;                // ls buffers: kColLs + 32 buf + 16 tile, 16 columns each
-  static constexpr uint32_t kColA = 320;                 // A stages start
+  static constexpr uint32_t kColLs = 256;                // mini-GEMM A operand (per-pixel constants): 8 columns per tile
+  static constexpr uint32_t kColA = 272;                 // A stages start (the mini-GEMM writes ls into a stage's lo half)
   static constexpr int kTail = 2 * kLsTile + kAC * 16;   // chunk tail: B1 | B2 (mini-GEMM operands) | IH records
 };
 
@@ -151,6 +150,11 @@ __device__ __forceinline__ void tmem_st16(uint32_t addr, const uint32_t (&v)[16]
   asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(addr),
                "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
                "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t addr, uint32_t v0, uint32_t v1, uint32_t v2, uint32_t v3, uint32_t v4, uint32_t v5,
+                                         uint32_t v6, uint32_t v7) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(addr), "r"(v0), "r"(v1), "r"(v2), "r"(v3),
+               "r"(v4), "r"(v5), "r"(v6), "r"(v7) : "memory");
 }
 __device__ __forceinline__ void tmem_ld8(uint32_t addr, float (&v)[8]) {
   uint32_t r[8];
@@ -259,8 +263,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   const uint32_t lbo = (uint32_t)(N / 8) * 128, sbo = 128;
 
   unsigned char* stage_base = smem_raw;
-  unsigned char* apix = smem_raw + align_up((size_t)kSB * chunk_bytes, 1024);                    // [2 tiles][kApixTile]
-  float* lev = reinterpret_cast<float*>(apix + (C::kLsOnTensor ? 2 * kApixTile : 0));            // [2 groups][L][256]
+  float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [2 groups][L][256]
   float* dsm = lev + 2 * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
   uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + 2 * (size_t)n_levels * NE);
   uint64_t* b_full = bars;                 // [kSB]
@@ -269,9 +272,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   uint64_t* a_empty = a_full + 2 * kSA;    // [kSA]
   uint64_t* d_full = a_empty + kSA;
   uint64_t* d_empty = d_full + 1;
-  uint64_t* ls_full = d_empty + 1;         // [2 buffers][2 tiles]
-  uint64_t* ls_empty = ls_full + 4;        // [2 buffers][2 tiles]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ls_empty + 4);
+  uint64_t* ls_full = d_empty + 1;         // [kSA][2 tiles]
+  uint64_t* apix_full = ls_full + 2 * kSA; // [2 tiles]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(apix_full + 2);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
@@ -280,7 +283,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 2); }
     mbar_init(d_full, 2);
     mbar_init(d_empty, kProducerWarps);
-    for (int b = 0; b < 4; ++b) { mbar_init(&ls_full[b], 1); mbar_init(&ls_empty[b], 4); }
+    for (int b = 0; b < 2 * kSA; ++b) mbar_init(&ls_full[b], 1);
+    mbar_init(&apix_full[0], 4); mbar_init(&apix_full[1], 4);
     fence_barrier_init();
   }
   if (warp == kProducerWarps) {
@@ -300,23 +304,6 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   split_pixel(ok ? rprime[j] : 0.0, q.jx, q.lx, q.fx);
   split_pixel(ok ? rprime[pix_stride + j] : 0.0, q.jy, q.ly, q.fy);
   split_pixel(ok ? rprime[2 * pix_stride + j] : 0.0, q.jz, q.lz, q.fz);
-  if (C::kLsOnTensor && warp < kProducerWarps / 2) {
-    // A operand of the mini-GEMM, row = pixel, K = 16 halves (UMMA K-major, no swizzle; LBO 2048, SBO 128):
-    //   core column 0 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 1, 0}, core column 1 = lo of the same.
-    const float v[7] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz, 1.0f};
-    __align__(16) __half hi[8], lo[8];
-#pragma unroll
-    for (int t = 0; t < 8; ++t) {
-      const float x = t < 7 ? v[t] : 0.f;
-      hi[t] = __float2half_rn(x);
-      lo[t] = __float2half_rn(x - __half2float(hi[t]));
-    }
-    const int m = slot & 127;
-    unsigned char* row = apix + (size_t)(slot >> 7) * kApixTile + (size_t)(m >> 3) * 128 + (size_t)(m & 7) * 16;
-    *reinterpret_cast<int4*>(row) = *reinterpret_cast<const int4*>(hi);
-    *reinterpret_cast<int4*>(row + 2048) = *reinterpret_cast<const int4*>(lo);
-    fence_proxy_async_smem();                              // generic-proxy writes -> async-proxy (tensor core) reads
-  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -328,6 +315,25 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const int group = warp >> 3, tile = (warp >> 2) & 1;
     const int ptid = tid;                                  // 0..511 over both groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
+    if (C::kLsOnTensor && group == 0) {
+      // A operand of the mini-GEMM in TMEM, row = pixel, K = 16 halves in 8 columns:
+      //   columns 0-3 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 1, 0}, columns 4-7 = lo of the same.
+      const float v[7] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz, 1.0f};
+      __align__(16) __half hi[8], lo[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const float x = u < 7 ? v[u] : 0.f;
+        hi[u] = __float2half_rn(x);
+        lo[u] = __float2half_rn(x - __half2float(hi[u]));
+      }
+      const uint32_t* hw = reinterpret_cast<const uint32_t*>(hi);
+      const uint32_t* lw = reinterpret_cast<const uint32_t*>(lo);
+      tmem_st8(tmem_base + lane_field + C::kColLs + (uint32_t)tile * 8, hw[0], hw[1], hw[2], hw[3], lw[0], lw[1], lw[2], lw[3]);
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&apix_full[tile]);
+    }
     float* mylev = lev + (size_t)group * n_levels * kTilePixels + slot;
     int next_epi = 0, next_due = n_chunks;                 // epilogue e is due once this group produced a chunk of collect e + 1
     int sa = group, sb = group;                            // this group's chunks: n = group, group + 2, ...
@@ -336,9 +342,12 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       const bool have = n < total;
       if (have) {
         if (tid == 0) TR(0, 0);
-        mbar_wait(&a_empty[sa], pa ^ 1);
-        if (tid == 0) TR(0, 1);
-        mbar_wait(&b_full[sb], pb);
+        if constexpr (C::kLsOnTensor) {
+          // ls_full(n) also implies that the MMAs which last read this A stage have completed (same issuer, in order)
+          mbar_wait2(&b_full[sb], pb, &ls_full[2 * sa + tile], pa);
+        } else {
+          mbar_wait2(&a_empty[sa], pa ^ 1, &b_full[sb], pb);
+        }
         tc_fence_after();
         if (tid == 0) TR(0, 2);
         const int4* rec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes);
@@ -359,15 +368,10 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
             tmem_st16(a_col + C::kColsHalf + h * 16, lo);
           }
         } else {
-          // small phase part of this chunk (minus 2 pi) from the mini-GEMM, then release its TMEM buffer
+          // small phase part of this chunk (minus 2 pi): the mini-GEMM left it in the lo half of this A stage
           float ls[16];
-          mbar_wait(&ls_full[2 * group + tile], (uint32_t)((n >> 1) & 1));
-          tc_fence_after();
-          tmem_ld16(tmem_base + lane_field + C::kColLs + (uint32_t)(group * 32 + tile * 16), ls);
+          tmem_ld16(a_col + C::kColsHalf, ls);
           tmem_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&ls_empty[2 * group + tile]);
           const int4* ihrec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes + 2 * kLsTile);
           uint32_t hi[16], lo[16];                         // 16 antennas -> 16 packed (cos, sin) columns
 #pragma unroll
@@ -480,26 +484,32 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
       // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) - 2 pi for the 16
-      // antennas of chunk m into TMEM buffer m & 1; issued two chunks ahead of the main MMAs of chunk m.
+      // antennas of chunk m, written into the lo half of A stage m % kSA two chunks ahead of the main MMAs of
+      // chunk m. The stage was last read by the main MMAs of chunk m - kSA, issued earlier by this same thread:
+      // the tensor pipe executes one thread's MMAs in order, so no barrier is needed to reuse the columns, and
+      // ls_full(m) tells the producers both "ls is there" and "the stage is free".
       const uint32_t idesc_ls = (1u << 4) | ((uint32_t)(kAC >> 3) << 17) | ((128u >> 4) << 24);
       const uint64_t desc_ls0 = make_b_desc(smem_u32(stage_base) + 2 * half_bytes, 2 * 128, 128);
-      const uint64_t desc_ap = make_b_desc(smem_u32(apix) + t * kApixTile, 2048, 128);
-      int sbm = 0;
+      const uint32_t a_pix = tb + C::kColLs + (uint32_t)t * 8;
+      int sbm = 0, sam = 0;
       uint32_t pbm = 0;
-      auto issue_mini = [&](int m) {
-        if (m >= 2) mbar_wait2(&b_full[sbm], pbm, &ls_empty[2 * (m & 1) + t], (uint32_t)(((m >> 1) - 1) & 1));
-        else mbar_wait(&b_full[sbm], pbm);
+      auto issue_mini = [&]() {
+        mbar_wait(&b_full[sbm], pbm);
         tc_fence_after();
         const uint64_t b1 = desc_ls0 + (uint64_t)((uint32_t)sbm * chunk16), b2 = b1 + (uint64_t)(kLsTile >> 4);
-        const uint32_t dl = tb + C::kColLs + (uint32_t)((m & 1) * 32 + t * 16);
-        mma_ss_f16(dl, desc_ap, b1, idesc_ls, 0u);         // A_hi B_hi + A_lo B_hi
-        mma_ss_f16(dl, desc_ap, b2, idesc_ls, 1u);         // A_hi B_lo
-        tc_commit(&ls_full[2 * (m & 1) + t]);
+        const uint32_t dl = tb + kColA + (uint32_t)sam * kColsStage + (uint32_t)t * 2 * C::kColsHalf + C::kColsHalf;
+        mma_ts<BB_TC_FP16>(dl, a_pix, b1, idesc_ls, 0u);   // A_hi B_hi + A_lo B_hi
+        mma_ts<BB_TC_FP16>(dl, a_pix, b2, idesc_ls, 1u);   // A_hi B_lo
+        tc_commit(&ls_full[2 * sam + t]);
         if (++sbm == kSB) { sbm = 0; pbm ^= 1; }
+        if (++sam == kSA) sam = 0;
       };
       if (C::kLsOnTensor) {
-        if (total > 0) issue_mini(0);
-        if (total > 1) issue_mini(1);
+        static_assert(!C::kLsOnTensor || kSA >= 3, "the mini-GEMM runs two chunks ahead");
+        mbar_wait(&apix_full[t], 0);
+        tc_fence_after();
+        if (total > 0) issue_mini();
+        if (total > 1) issue_mini();
       }
       for (int e = 0; e < n_collects; ++e) {
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
@@ -507,7 +517,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         for (int c = 0; c < n_chunks; ++c, ++n) {
           if (t == 0) TR(1, 0);
           if (C::kLsOnTensor) {
-            if (n + 2 < total) issue_mini(n + 2);          // (its b_full wait covered chunk n two iterations ago)
+            if (n + 2 < total) issue_mini();               // chunk n + 2 (its b_full wait covered chunk n two iterations ago)
             if (t == 0) TR(1, 1);
             mbar_wait(&a_full[2 * sa + t], pa);
           } else {
@@ -526,7 +536,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
               const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
               mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
             }
-          tc_commit(&a_empty[sa]);
+          if (!C::kLsOnTensor) tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
           if (t == 0) TR(1, 3);
@@ -698,8 +708,7 @@ template <int MODE>
 int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + (C::kLsOnTensor ? 2 * kApixTile : 0) +
-                      2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 3 * C::kSA + 10) * 8 + 16 + 1024;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) +                       2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 4) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
