@@ -335,6 +335,13 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       if (lane == 0) mbar_arrive(&apix_full[tile]);
     }
     float* mylev = lev + (size_t)group * n_levels * kTilePixels + slot;
+    int woff[4];                                           // this thread's share of a collect's [level][NE] weight block
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = ptid + u * kProducerWarps * 32;
+      const int l = i / NE, k = i - l * NE;
+      woff[u] = i < n_levels * NE ? l * n_eig_pad + eig_offset + k : -1;
+    }
     int next_epi = 0, next_due = n_chunks;                 // epilogue e is due once this group produced a chunk of collect e + 1
     int sa = group, sb = group;                            // this group's chunks: n = group, group + 2, ...
     uint32_t pa = 0, pb = 0;                               // phase parities of the A / B stage rings
@@ -403,16 +410,11 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         float wnext[4];                                    // prefetch the weights of collect e + 1 (<= 2048 floats)
         if (e + 1 < n_collects) {
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int i = ptid + u * kProducerWarps * 32;
-            if (i < n_levels * NE) {
-              const int l = i / NE, k = i - l * NE;
-              wnext[u] = weights[(size_t)(e + 1) * weight_stride + (size_t)l * n_eig_pad + eig_offset + k];
-            }
-          }
+          for (int u = 0; u < 4; ++u)
+            if (woff[u] >= 0) wnext[u] = weights[(size_t)(e + 1) * weight_stride + woff[u]];
         }
         const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128);
-        float pw[kMaxNE / 2];                              // this group's eigenpair octets: g = group, group + 2, ...
+        float2 pw[kMaxNE / 4];                             // |E|^2 of this group's eigenpair octets g = group, group + 2, ...
 #pragma unroll
         for (int gg = 0; gg < kMaxNE / 16; ++gg) {
           const int g = 2 * gg + group;
@@ -422,42 +424,39 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
             tmem_ld8(d_col + NE + g * 8, im);
             tmem_wait_ld();
 #pragma unroll
-            for (int t = 0; t < 8; ++t) pw[gg * 8 + t] = re[t] * re[t] + im[t] * im[t];
+            for (int t = 0; t < 4; ++t) {
+              const float2 r2 = make_float2(re[2 * t], re[2 * t + 1]), i2 = make_float2(im[2 * t], im[2 * t + 1]);
+              pw[gg * 4 + t] = __ffma2_rn(i2, i2, __fmul2_rn(r2, r2));
+            }
           } else {
 #pragma unroll
-            for (int t = 0; t < 8; ++t) pw[gg * 8 + t] = 0.f;
+            for (int t = 0; t < 4; ++t) pw[gg * 4 + t] = make_float2(0.f, 0.f);
           }
         }
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(d_empty);               // D may be overwritten by the next collect
-        for (int l = 0; l < n_levels; ++l) {
-          float sacc = 0.f;
+        for (int l = 0; l < n_levels; ++l) {               // a3: I_l += sum_k D[l,k] |E_k|^2 (packed pairs over k)
+          float2 sacc = make_float2(0.f, 0.f);
 #pragma unroll
           for (int gg = 0; gg < kMaxNE / 16; ++gg) {
             const int g = 2 * gg + group;
             if (g * 8 < NE) {
               const float4* dl = reinterpret_cast<const float4*>(dcur + (size_t)l * NE + g * 8);
               const float4 w0 = dl[0], w1 = dl[1];
-              sacc = fmaf(w0.x, pw[gg * 8], sacc);
-              sacc = fmaf(w0.y, pw[gg * 8 + 1], sacc);
-              sacc = fmaf(w0.z, pw[gg * 8 + 2], sacc);
-              sacc = fmaf(w0.w, pw[gg * 8 + 3], sacc);
-              sacc = fmaf(w1.x, pw[gg * 8 + 4], sacc);
-              sacc = fmaf(w1.y, pw[gg * 8 + 5], sacc);
-              sacc = fmaf(w1.z, pw[gg * 8 + 6], sacc);
-              sacc = fmaf(w1.w, pw[gg * 8 + 7], sacc);
+              sacc = __ffma2_rn(make_float2(w0.x, w0.y), pw[gg * 4], sacc);
+              sacc = __ffma2_rn(make_float2(w0.z, w0.w), pw[gg * 4 + 1], sacc);
+              sacc = __ffma2_rn(make_float2(w1.x, w1.y), pw[gg * 4 + 2], sacc);
+              sacc = __ffma2_rn(make_float2(w1.z, w1.w), pw[gg * 4 + 3], sacc);
             }
           }
-          mylev[(size_t)l * kTilePixels] += sacc;
+          mylev[(size_t)l * kTilePixels] += sacc.x + sacc.y;
         }
         if (e + 1 < n_collects) {
           float* dnext = dsm + (size_t)((e + 1) & 1) * n_levels * NE;
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int i = ptid + u * kProducerWarps * 32;
-            if (i < n_levels * NE) dnext[i] = wnext[u];
-          }
+          for (int u = 0; u < 4; ++u)
+            if (woff[u] >= 0) dnext[ptid + u * kProducerWarps * 32] = wnext[u];
         }
       }
       if (!have) break;
