@@ -309,6 +309,24 @@ def run_ours(args):
         glue = {"gram_ms_per_collect": t3["gram_ms"] / ncol, "eig_ms_per_collect": t3["eig_ms"] / ncol,
                 "collects_timed": ncol, "precision": "f64", "solver": "cusolverDnZhegvd"}
 
+    # ---- the other kernel variants on the same device-resident inputs (north_star: compare them) ----
+    others = {}
+    if rank == 0 and not args.no_compare:
+        for v in ("fp32", "tf32x3", "fp16x3"):
+            if v == args.variant:
+                continue
+            sv = binding.StandardSynthesis(ctx, DM.from_numpy(pix, np.float64, dev), L, v)
+            for rep in range(3):                                  # 2 warm-up passes, 1 timed
+                if rep == 2:
+                    tb = sv.timings()
+                for it in dev_items:
+                    sv.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
+                sv.flush()
+                flush_buf.zero_()
+            ms = sv.timings()["synth_ms"] - tb["synth_ms"]
+            others[v] = {"synth_ms_per_step": ms, "terms_per_s": terms_step / (ms * 1e-3)}
+            del sv
+
     if rank != 0:
         return
     line = {
@@ -329,6 +347,7 @@ def run_ours(args):
         "kernel_ms": {"synth_ms_per_step": synth_ms / args.steps, "prep_ms_per_step": prep_ms / args.steps,
                       "synth_launches": int(synth_launches)},
         "glue": glue,
+        "other_variants": others,
     }
     peak = FP32_PEAK_TFLOPS
     bound = "alu"
@@ -343,6 +362,10 @@ def run_ours(args):
                         "flops_per_launch": flops_per_launch, "avg_launch_ms": avg_launch_ms,
                         "peak_basis": ("148 SM x 128 FP32 lanes x 2 x 1.965 GHz (derived, DESIGN.md)" if bound == "alu" else
                                        ("1.0" if args.variant == "fp16x3" else "0.5") + " x measured bf16 burst (MEASURED_PEAKS.json); useful flops = 8/term, issued = 24/term")}
+    if bound == "tensor":
+        # the split-precision scheme issues 3 tensor passes per useful one: 24 flops per term on the pipe
+        line["roofline"]["issued_tflops"] = 3.0 * achieved_tflops
+        line["roofline"]["issued_frac"] = 3.0 * achieved_tflops / peak
     if clocks.get("sm_mhz"):
         line["roofline"]["frac_at_observed_clock"] = achieved_tflops / (peak * clocks["sm_mhz"] / SM_MAX_MHZ) if bound == "alu" else None
     if args.probe:
@@ -361,7 +384,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp32"))
+    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp16x3"), choices=["fp32", "tf32x3", "fp16x3"])
+    ap.add_argument("--no-compare", action="store_true", help="skip the short timing of the other two variants")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--probe", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

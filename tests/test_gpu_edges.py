@@ -145,3 +145,38 @@ def test_empty_image(bb, ctx):
     s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
     s.flush()
     assert s.get(0).shape == (0,)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("extent,wavelength,fov", [
+    (60000.0, 1.0, 0.35),      # 120 km array at 1 m: |p'| up to 1e5 wavelengths, phases of ~3e4 turns
+    (35000.0, 2.5, 0.26),      # config-4-like extremes
+    (300.0, 15.0, 1.0)])       # compact array, pixels all over the hemisphere (|r - r_c| ~ 1)
+def test_phase_generator_range(bb, ctx, oracle, variant, extent, wavelength, fov):
+    """The range reduction (fp64 in the FP32 kernel, integer + tensor-core mini-GEMM in the tensor kernels) must
+    hold its precision for very long baselines and for pixel sets far from the field centre."""
+    c = random_case(4242, 96, 24, 3, 1500, extent=extent, fov=min(fov, 0.7))
+    if fov >= 1.0:             # unit vectors over a wide cap instead of a small tangent patch
+        rng = np.random.default_rng(7)
+        v = rng.normal(size=(1500, 3)); v[:, 2] = np.abs(v[:, 2]) + 0.2
+        c["pix"] = np.asfortranarray(v / np.linalg.norm(v, axis=1, keepdims=True))
+    ref = oracle.synth(c["B"], c["D"], c["xyz"], c["pix"], wavelength)
+    s = bb.StandardSynthesis(ctx, c["pix"], 3, variant)
+    s.collect_eig(c["B"], c["D"], c["xyz"], wavelength)
+    assert_parity(s.images(), ref, "%s extent %g" % (variant, extent))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_column_magnitudes_span_many_decades(bb, ctx, oracle, variant):
+    """Eigenvector columns of very different size (and one all-zero column): the FP16 variant rescales each
+    column by a power of two and folds it into the weights; the result must not depend on the magnitudes."""
+    c = random_case(99, 80, 12, 2, 700)
+    scale = np.array([1e-9, 1e-6, 1e-3, 1.0, 37.0, 1e3, 1e5, 3e-12, 0.0, 2.0, 1e-1, 5e6], dtype=np.float64)
+    B = (c["B"].astype(np.complex128) * scale[None, :]).astype(np.complex64)
+    D = c["D"].astype(np.float64)
+    D[:, scale > 0] /= scale[scale > 0][None, :] ** 2          # keep every column's contribution O(1)
+    B, D = np.asfortranarray(B), np.asfortranarray(D.astype(np.float32))
+    ref = oracle.synth(B, D, c["xyz"], c["pix"], c["wavelength"])
+    s = bb.StandardSynthesis(ctx, c["pix"], 2, variant)
+    s.collect_eig(B, D, c["xyz"], c["wavelength"])
+    assert_parity(s.images(), ref, variant)
