@@ -47,7 +47,7 @@ def measured_peaks():
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index=0, period=0.05):
+    def __init__(self, index=0, period=0.002):
         super().__init__(daemon=True)
         self.index, self.period, self.samples, self.reasons, self.max_mhz = index, period, [], set(), None
         self._stop_ev = threading.Event()
@@ -366,10 +366,15 @@ def run_ours(args):
         # the split-precision scheme issues 3 tensor passes per useful one: 24 flops per term on the pipe
         line["roofline"]["issued_tflops"] = 3.0 * achieved_tflops
         line["roofline"]["issued_frac"] = 3.0 * achieved_tflops / peak
+        sus = mp.get("bf16_tflops_sustained")
+        if sus:                                              # the power-capped figure (cuBLAS bf16 back to back for seconds)
+            line["roofline"]["issued_frac_of_sustained_peak"] = 3.0 * achieved_tflops / (sus * (1.0 if args.variant == "fp16x3" else 0.5))
     if clocks.get("sm_mhz"):
         line["roofline"]["frac_at_observed_clock"] = achieved_tflops / (peak * clocks["sm_mhz"] / SM_MAX_MHZ) if bound == "alu" else None
     if args.probe:
-        line["probe"] = {k: ctx.probe_peak(i)[0] for i, k in enumerate(["ffma_per_s", "ffma2_fma_per_s", "mufu_per_s", "dfma_per_s"])}
+        line["probe"] = {k: ctx.probe_peak(i)[0] for i, k in enumerate(
+            ["ffma_per_s", "ffma2_fma_per_s", "mufu_per_s", "dfma_per_s", "dfma_chains_alone_per_s", "dfma_chains_under_mma_per_s",
+             "imad_chains_alone_per_s", "imad_chains_under_mma_per_s"])}
     if world == 1 and not args.no_cpu_baseline:
         from oracle import bluebild_oracle as oracle      # cpu_baseline leg: the one place bench.py runs the oracle
         oracle.build()

@@ -116,7 +116,10 @@ int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, con
 /* ---- peak probes (measurement support) --------------------------------
  * kind: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2), 2 = MUFU sin+cos, 3 = DFMA. Runs a register-only
  * loop on every SM and returns operations per second in *ops_per_s (FMA counted as 1 op per
- * lane; kind 1 counts 2 per lane-instruction) and the kernel time in *ms. */
+ * lane; kind 1 counts 2 per lane-instruction) and the kernel time in *ms.
+ * kind 4/5 = DFMA chains on 8 warps per SM without / with a concurrent tcgen05.mma stream on the
+ * same SM, kind 6/7 = the same for IMAD: *ms is the slowest warp's clock64 span at the nominal
+ * maximum clock, *ops_per_s the lane-operations over that span (interference probe). */
 int bb_probe_peak(bb_ctx* ctx, int kind, double* ops_per_s, double* ms);
 
 const char* bb_status_string(int status);

@@ -180,3 +180,15 @@ def test_column_magnitudes_span_many_decades(bb, ctx, oracle, variant):
     s = bb.StandardSynthesis(ctx, c["pix"], 2, variant)
     s.collect_eig(B, D, c["xyz"], c["wavelength"])
     assert_parity(s.images(), ref, variant)
+
+
+def test_interference_probe(bb, ctx):
+    """bb_probe_peak kinds 4-7: fp64 FMA chains slow down under a concurrent tcgen05.mma stream on the same SM
+    (the reason the tensor variants reduce phases in integer arithmetic), integer multiply-adds do not."""
+    dfma_alone, _ = ctx.probe_peak(4)
+    dfma_mma, _ = ctx.probe_peak(5)
+    imad_alone, _ = ctx.probe_peak(6)
+    imad_mma, _ = ctx.probe_peak(7)
+    assert min(dfma_alone, dfma_mma, imad_alone, imad_mma) > 0
+    assert dfma_mma < 0.8 * dfma_alone, (dfma_alone, dfma_mma)
+    assert imad_mma > 0.8 * imad_alone, (imad_alone, imad_mma)
