@@ -81,6 +81,21 @@ int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavel
                      const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz,
                      int ldxyz, const double* intervals, int ld_int);
 
+/* ---- collect_ex: Algorithm 1 with N_f filters (Alg. 1 l.6-7) and the Gram choice ----
+ * filters: n_filters (1..BB_MAX_FILTERS) entries, HOST pointer, BB_FILTER_LSQ (d = lambda, Eq. 14/20) or
+ * BB_FILTER_STD (d = 1, the "Standardized" image). The handle's n_levels must equal n_intervals * n_filters
+ * with n_intervals = n_levels / n_filters rows in `intervals`; image index = filter * n_intervals + interval
+ * (the B^(n_i, n_f) of Alg. 1 l.9). gram_mode BB_GRAM_SINC is Eq. 11/24; BB_GRAM_IDENTITY sets G := I, the
+ * eigendecomposition of the dirty image (Eq. 38-40, App. A). All else as bb_synth_collect,
+ * which is collect_ex with one LSQ filter and the sinc Gram. */
+enum { BB_FILTER_LSQ = 0, BB_FILTER_STD = 1 };
+enum { BB_GRAM_SINC = 0, BB_GRAM_IDENTITY = 1 };
+#define BB_MAX_FILTERS 8
+int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength,
+                        const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz,
+                        int ldxyz, const double* intervals, int ld_int, int n_filters,
+                        const int* filters, int gram_mode);
+
 /* ---- collect_eig: the hot path only (Algorithm 2 + Alg. 1 line 9, Eq. 15, 20) ---------------
  * I_l(r_j) += sum_k D[l,k] | sum_i conj(B_ik) exp(+j 2 pi <xyz_i, r_j> / wavelength) |^2
  *   B   n_ant x n_eig complex64 (= W V), ld ldb

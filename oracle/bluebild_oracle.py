@@ -114,7 +114,12 @@ def select(lam, V, n_eig):
 
 
 def level_weights(lam, intervals, filt="lsq"):
-    """D[l,k] for closed intervals [min_l, max_l] (reading Q7), LSQ (d = lambda) or STD (d = 1)."""
+    """D[l,k] for closed intervals [min_l, max_l] (reading Q7), LSQ (d = lambda) or STD (d = 1).
+    `filt` may also be a sequence of filters (Alg. 1 l.6: N_f filters): the blocks are stacked, row
+    f * N_i + i belonging to (filter f, interval i) = B^(n_i, n_f) of Alg. 1 l.9."""
+    if not isinstance(filt, str):
+        return np.vstack([level_weights(lam, intervals, f) for f in filt])
+    assert filt in ("lsq", "std")
     lam = np.asarray(lam, dtype=np.float64)
     intervals = np.asarray(intervals, dtype=np.float64).reshape(-1, 2)
     inside = (lam[None, :] >= intervals[:, :1]) & (lam[None, :] <= intervals[:, 1:])

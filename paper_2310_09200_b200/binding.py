@@ -20,10 +20,12 @@ BB_OK = 0
 VARIANT_FP32 = 0
 VARIANT_TF32X3 = 1
 VARIANT_FP16X3 = 2
+FILTERS = {"lsq": 0, "std": 1}
+GRAM_MODES = {"sinc": 0, "identity": 1}
 _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_FP16X3, 0: 0, 1: 1, 2: 2}
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
-           "bb_synth_collect", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
+           "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_launches", "bb_eig", "bb_probe_peak", "bb_status_string", "bb_version"]
 
 _lib = None
@@ -55,6 +57,7 @@ def load_library(path: str = LIB_PATH):
         "bb_synth_destroy": ([vp], i32),
         "bb_synth_reset": ([vp], i32),
         "bb_synth_collect": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32], i32),
+        "bb_synth_collect_ex": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32, i32, vp, i32], i32),
         "bb_synth_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
         "bb_synth_flush": ([vp], i32),
         "bb_synth_get": ([vp, i32, vp], i32),
@@ -172,14 +175,24 @@ class StandardSynthesis:
     def reset(self):
         _check(_lib.bb_synth_reset(self._h), "bb_synth_reset")
 
-    def collect(self, S, W, xyz, wavelength, n_eig, intervals):
+    def collect(self, S, W, xyz, wavelength, n_eig, intervals, filters=None, gram="sinc"):
+        """Algorithm 1. filters: None (one LSQ filter) or a sequence of "lsq" / "std"; the handle's n_levels must be
+        len(filters) * len(intervals) and image f * n_intervals + i belongs to (filter f, interval i).
+        gram: "sinc" (Eq. 11) or "identity" (dirty-image eigendecomposition)."""
         keep = []
         Sp, n_beam, _, lds = _marshal(S, np.complex64, keep)
         Wp, _, _, ldw = _marshal(W, np.complex64, keep)
         Xp, n_ant, _, ldx = _marshal(xyz, np.float64, keep)
         Ip, _, _, ldi = _marshal(intervals, np.float64, keep)
-        _check(_lib.bb_synth_collect(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
-                                     Ip, ldi), "bb_synth_collect")
+        if filters is None and gram == "sinc":
+            _check(_lib.bb_synth_collect(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
+                                         Ip, ldi), "bb_synth_collect")
+            return
+        kinds = [FILTERS[f] for f in (filters or ["lsq"])]
+        arr = (ctypes.c_int * len(kinds))(*kinds)
+        _check(_lib.bb_synth_collect_ex(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
+                                        Ip, ldi, len(kinds), ctypes.cast(arr, ctypes.c_void_p), GRAM_MODES[gram]),
+               "bb_synth_collect_ex")
 
     def collect_eig(self, B, D, xyz, wavelength):
         keep = []

@@ -354,8 +354,26 @@ extern "C" int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wa
 extern "C" int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W,
                                 int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
                                 const double* intervals, int ld_int) {
-  if (!s || !S || !xyz || !intervals || n_ant < 1 || n_beam < 1 || n_eig < 1 || n_eig > n_beam ||
-      n_beam > BB_MAX_BEAMS || !(wavelength > 0.0) || lds < n_beam || ldxyz < n_ant || ld_int < s->n_levels ||
+  const int lsq = BB_FILTER_LSQ;
+  return bb_synth_collect_ex(s, n_ant, n_beam, n_eig, wavelength, W, ldw, S, lds, xyz, ldxyz, intervals, ld_int, 1, &lsq,
+                             BB_GRAM_SINC);
+}
+
+extern "C" int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W,
+                                   int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
+                                   const double* intervals, int ld_int, int n_filters, const int* filters, int gram_mode) {
+  if (!s || !S || !xyz || !intervals || !filters || n_filters < 1 || n_filters > BB_MAX_FILTERS ||
+      s->n_levels % n_filters != 0 || (gram_mode != BB_GRAM_SINC && gram_mode != BB_GRAM_IDENTITY))
+    return BB_EINVAL;
+  const int n_intervals = s->n_levels / n_filters;
+  FilterList fl{};
+  fl.n = n_filters;
+  for (int f = 0; f < n_filters; ++f) {
+    if (filters[f] != BB_FILTER_LSQ && filters[f] != BB_FILTER_STD) return BB_EINVAL;
+    fl.kind[f] = filters[f];
+  }
+  if (n_ant < 1 || n_beam < 1 || n_eig < 1 || n_eig > n_beam ||
+      n_beam > BB_MAX_BEAMS || !(wavelength > 0.0) || lds < n_beam || ldxyz < n_ant || ld_int < n_intervals ||
       (W && ldw < n_ant) || (!W && n_beam != n_ant) || n_ant > (1 << 20))
     return BB_EINVAL;
   BB_CUDA(cudaSetDevice(s->ctx->device));
@@ -368,14 +386,14 @@ extern "C" int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, d
   const bb_c32* Wd = st.put(W, n_ant, n_beam, ldw, &ldw2);
   const bb_c32* Sd = st.put(S, n_beam, n_beam, lds, &lds2);
   const double* Xd = st.put(xyz, n_ant, 3, ldxyz, &ldx2);
-  const double* Id = st.put(intervals, s->n_levels, 2, ld_int, &ldi2);
+  const double* Id = st.put(intervals, n_intervals, 2, ld_int, &ldi2);
   if ((rc = st.commit()) != BB_OK) return rc;
   bb_c32* Bd = s->glue_B + (size_t)slot * n_ant * n_eig;
   double* lam = s->glue_lambda + (size_t)slot * n_eig;
   float* Dd = s->glue_D + (size_t)slot * s->n_levels * n_eig;
   cudaEvent_t e0 = get_event(s), e1 = get_event(s), e2 = get_event(s), e3 = get_event(s);
   rc = bb_glue_eig(s->ctx->glue, s->ctx->stream, n_ant, n_beam, n_eig, wavelength, Wd, ldw2, Sd, lds2, Xd, ldx2, lam,
-                   Bd, e0, e1, e2, e3);
+                   Bd, e0, e1, e2, e3, gram_mode);
   if (rc != BB_OK) {
     s->free_ev.push_back(e0); s->free_ev.push_back(e1); s->free_ev.push_back(e2); s->free_ev.push_back(e3);
     return rc;
@@ -383,7 +401,7 @@ extern "C" int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, d
   s->spans.push_back(Span{e0, e1, T_GRAM});
   s->spans.push_back(Span{e2, e3, T_EIG});
   s->launches += 6;  // gram, symmetrise/convert, select, cast kernels of glue.cu (library calls not counted)
-  if ((rc = bb_launch_level_weights(lam, n_eig, Id, ldi2, s->n_levels, Dd, s->n_levels, s->ctx->stream)) != BB_OK) return rc;
+  if ((rc = bb_launch_level_weights(lam, n_eig, Id, ldi2, n_intervals, fl, Dd, s->n_levels, s->ctx->stream)) != BB_OK) return rc;
   s->launches += 1;
   return enqueue_prepared(s, n_ant, n_eig, wavelength, Bd, n_ant, Dd, s->n_levels, Xd, ldx2);
 }

@@ -73,12 +73,19 @@ __global__ void narrow_kernel(const cuDoubleComplex* __restrict__ src, int rows,
 }
 
 __global__ void level_weights_kernel(const double* __restrict__ lam, int n_eig, const double* __restrict__ iv, int ld_int,
-                                     int n_levels, float* __restrict__ D, int ldd) {
+                                     int n_intervals, FilterList filters, float* __restrict__ D, int ldd) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x, l = blockIdx.y;
-  if (k < n_eig && l < n_levels) {
+  if (k < n_eig && l < n_intervals * filters.n) {
+    const int f = l / n_intervals, i = l - f * n_intervals;
     const double x = lam[k];
-    D[l + (size_t)k * ldd] = (x >= iv[l] && x <= iv[l + ld_int]) ? (float)x : 0.f;
+    const float d = filters.kind[f] == BB_FILTER_STD ? 1.f : (float)x;      // Alg. 1 l.7: LSQ d = lambda, STD d = 1
+    D[l + (size_t)k * ldd] = (x >= iv[i] && x <= iv[i + ld_int]) ? d : 0.f;
   }
+}
+
+__global__ void identity_kernel(cuDoubleComplex* __restrict__ a, int n) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y;
+  if (r < n) a[r + (size_t)c * n] = make_cuDoubleComplex(r == c ? 1.0 : 0.0, 0.0);
 }
 
 template <class T> int grow(T** p, size_t n) {
@@ -114,7 +121,7 @@ void bb_glue_destroy(GlueWork* g) {
 
 int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W,
                 int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz, double* lambda_dev, bb_c32* B_dev,
-                cudaEvent_t ev_gram0, cudaEvent_t ev_gram1, cudaEvent_t ev_eig0, cudaEvent_t ev_eig1) {
+                cudaEvent_t ev_gram0, cudaEvent_t ev_gram1, cudaEvent_t ev_eig0, cudaEvent_t ev_eig1, int gram_mode) {
   cublasSetStream(g->blas, st);
   cusolverDnSetStream(g->solver, st);
   if (n_ant > g->cap_ant || n_beam > g->cap_beam) {
@@ -134,9 +141,13 @@ int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, 
 
   // ---- a0: Gram
   if (ev_gram0) cudaEventRecord(ev_gram0, st);
-  gram_psi_kernel<<<dim3((n_ant + 127) / 128, n_ant), blk, 0, st>>>(xyz, ldxyz, n_ant, wavelength, W ? g->psi : g->g);
-  if (W) {
-    widen_kernel<<<dim3((n_ant + 127) / 128, n_beam), blk, 0, st>>>(W, ldw, n_ant, n_beam, g->w128);
+  if (W) widen_kernel<<<dim3((n_ant + 127) / 128, n_beam), blk, 0, st>>>(W, ldw, n_ant, n_beam, g->w128);
+  if (gram_mode == BB_GRAM_IDENTITY) {                    // G := I: eigendecomposition of the dirty image (Eq. 38-40)
+    identity_kernel<<<dim3((n_beam + 127) / 128, n_beam), blk, 0, st>>>(g->g, n_beam);
+  } else {
+    gram_psi_kernel<<<dim3((n_ant + 127) / 128, n_ant), blk, 0, st>>>(xyz, ldxyz, n_ant, wavelength, W ? g->psi : g->g);
+  }
+  if (W && gram_mode != BB_GRAM_IDENTITY) {
     if (cublasZgemm(g->blas, CUBLAS_OP_N, CUBLAS_OP_N, n_ant, n_beam, n_ant, &one, g->psi, n_ant, g->w128, n_ant, &zero,
                     g->t, n_ant) != CUBLAS_STATUS_SUCCESS ||
         cublasZgemm(g->blas, CUBLAS_OP_C, CUBLAS_OP_N, n_beam, n_beam, n_ant, &one, g->w128, n_ant, g->t, n_ant, &zero,
@@ -186,10 +197,10 @@ int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, 
   return BB_OK;
 }
 
-int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int, int n_levels,
-                            float* D_dev, int ldd, cudaStream_t st) {
-  level_weights_kernel<<<dim3((n_eig + 127) / 128, n_levels), 128, 0, st>>>(lambda_dev, n_eig, intervals_dev, ld_int,
-                                                                          n_levels, D_dev, ldd);
+int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int, int n_intervals,
+                            FilterList filters, float* D_dev, int ldd, cudaStream_t st) {
+  level_weights_kernel<<<dim3((n_eig + 127) / 128, n_intervals * filters.n), 128, 0, st>>>(lambda_dev, n_eig, intervals_dev,
+                                                                                          ld_int, n_intervals, filters, D_dev, ldd);
   BB_CUDA(cudaGetLastError());
   return BB_OK;
 }

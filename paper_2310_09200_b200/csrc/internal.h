@@ -91,8 +91,10 @@ void bb_glue_destroy(GlueWork* g);
 int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, double wavelength,
                 const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
                 double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
-                cudaEvent_t ev_eig0, cudaEvent_t ev_eig1);
+                cudaEvent_t ev_eig0, cudaEvent_t ev_eig1, int gram_mode = BB_GRAM_SINC);
+struct FilterList { int n; int kind[BB_MAX_FILTERS]; };
+// D[f * n_intervals + i, k] = d_f(lambda_k) [min_i <= lambda_k <= max_i]
 int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int,
-                            int n_levels, float* D_dev, int ldd, cudaStream_t st);
+                            int n_intervals, FilterList filters, float* D_dev, int ldd, cudaStream_t st);
 
 int bb_probe_run(int kind, int sm_count, cudaStream_t st, double* ops_per_s, double* ms);

@@ -152,3 +152,26 @@ def test_cfg5_multichannel_two_epochs_full_image(bb, ctx, wl, oracle, variant):
     for it in items:
         s.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
     assert_parity(s.images()[:, sub], ref, "cfg5")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("gram", ["sinc", "identity"])
+def test_collect_ex_filters_and_gram_mode(bb, ctx, oracle, variant, gram):
+    """N_f = 2 filters (STD, LSQ) x 2 intervals through bb_synth_collect_ex, with the sinc
+    Gram and with G := I (dirty-image eigendecomposition), against the oracle's Algorithm 1."""
+    from paper_2310_09200_b200 import workloads
+    w = workloads.make_workload(1)
+    ci = w.collect_inputs(0)
+    pix = w.pixels()
+    lam, _ = oracle.eig_stage(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, gram_identity=(gram == "identity"))
+    iv = workloads.choose_intervals(lam, 2)
+    ref = oracle.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, pix, filt=("std", "lsq"),
+                         gram_identity=(gram == "identity"))
+    s = bb.StandardSynthesis(ctx, pix, 4, variant)
+    s.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, filters=["std", "lsq"], gram=gram)
+    assert_parity(s.images(), ref, "%s %s" % (variant, gram))
+    # wrong level count for the filter list is rejected and leaves the images untouched
+    s3 = bb.StandardSynthesis(ctx, pix, 3, variant)
+    with pytest.raises(bb.BluebildError):
+        s3.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, filters=["std", "lsq"])
+    assert not s3.images().any()

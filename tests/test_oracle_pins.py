@@ -328,3 +328,48 @@ def test_select_largest_signed(oracle):
     V = np.arange(16.0).reshape(4, 4)
     l, v = oracle.select(lam, V, 2)
     assert np.array_equal(l, [3.0, 2.0]) and np.array_equal(v, V[:, [2, 3]])
+
+
+# ---------------------------------------------------------------------------------- filters
+@pytest.mark.parametrize("beamformed", [False, True])
+def test_P7_standardized_filter_sums_to_inverse_gram_form(oracle, beamformed):
+    """STD filter (d = 1) over ALL eigenpairs: sum_k |v_k^H a_W|^2 = a_W^H G^-1 a_W because the
+    G-orthonormal eigenvectors satisfy V V^H = G^-1 -- a linear solve, no eigensolver."""
+    rng = np.random.default_rng(41 + beamformed)
+    xyz, pix, wl = _tiny_case(rng, n_ant=12, n=12)
+    W = (rng.normal(size=(12, 5)) + 1j * rng.normal(size=(12, 5))) / 3.0 if beamformed else None
+    S = _random_sky_S(rng, xyz, wl, W=W)
+    nb = S.shape[0]
+    d = np.linalg.norm(xyz[:, None, :] - xyz[None, :, :], axis=-1)
+    Psi = np.sinc(2.0 * d / wl)
+    G = Psi if W is None else W.conj().T @ Psi @ W
+    A = steering(xyz, pix, wl)
+    aW = A if W is None else W.conj().T @ A
+    expect = np.real(np.sum(aW.conj() * np.linalg.solve(G, aW), axis=0))
+    img = oracle.collect(S, W, xyz, wl, nb, [[-1e9, 1e9]], pix, filt="std")[0]
+    assert np.allclose(img, expect, rtol=0, atol=1e-10 * expect.max())
+
+
+def test_P7_standardized_identity_gram_is_constant(oracle):
+    """G := I, W = I, STD filter, all eigenpairs: sum_k |v_k^H a|^2 = |a|^2 = N_ant at every pixel."""
+    rng = np.random.default_rng(43)
+    xyz, pix, wl = _tiny_case(rng, n_ant=9, n=8)
+    S = _random_sky_S(rng, xyz, wl)
+    img = oracle.collect(S, None, xyz, wl, 9, [[-1e9, 1e9]], pix, filt="std", gram_identity=True)[0]
+    assert np.allclose(img, 9.0, rtol=0, atol=1e-10)
+
+
+def test_filters_stack_as_interval_blocks(oracle):
+    """N_f filters (Alg. 1 l.6-12): image f * N_i + i is (filter f, interval i), each block equal to the
+    single-filter run; LSQ and STD blocks differ exactly by the eigenvalue weights."""
+    rng = np.random.default_rng(44)
+    xyz, pix, wl = _tiny_case(rng, n_ant=10, n=6)
+    S = _random_sky_S(rng, xyz, wl)
+    lam, B = oracle.eig_stage(S, None, xyz, wl, 6)
+    iv = [[lam[2] * 0.999, 2 * lam[0]], [0.0, lam[3] * 1.001]]
+    both = oracle.collect(S, None, xyz, wl, 6, iv, pix, filt=("std", "lsq"))
+    assert both.shape[0] == 4
+    assert np.array_equal(both[:2], oracle.collect(S, None, xyz, wl, 6, iv, pix, filt="std"))
+    assert np.array_equal(both[2:], oracle.collect(S, None, xyz, wl, 6, iv, pix, filt="lsq"))
+    D = oracle.level_weights(lam, iv, ("std", "lsq"))
+    assert np.array_equal(D[2:], D[:2] * lam[None, :])
