@@ -90,7 +90,9 @@ class ClockSampler(threading.Thread):
         if self.is_alive():
             self.join(timeout=2)
         med = float(np.median(self.samples)) if self.samples else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        lo = float(np.min(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_min_mhz": lo, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
 
 
 # ------------------------------------------------------------------------------------ workload
@@ -275,7 +277,7 @@ def run_ours(args):
 
     # ---- end-to-end arm: host buffers in, host images out, through the C ABI --------------------
     s2 = binding.StandardSynthesis(ctx, pix, L, args.variant)
-    out = np.empty((L, c.n_pix), dtype=np.float32)
+    out = torch.empty((L, c.n_pix), dtype=torch.float32, pin_memory=True).numpy()    # page-locked result buffer
 
     def step_e2e():
         for it in items:
