@@ -128,6 +128,21 @@ int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, con
            int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz, double* lambda_out,
            bb_c32* B_out, int ldb_out);
 
+/* ---- parameter estimation (Table 4 caption :593), device-side glue -------------
+ * lambda: n (1..BB_MAX_ESTIMATE) eigenvalues in any order, host or device (one collect's, or pooled from a
+ * subset of the data, e.g. from bb_eig). Both calls synchronise the context stream.
+ * bb_estimate_n_eig: the smallest m such that the m largest eigenvalues hold at least energy_fraction
+ *   (0 < f <= 1) of the sum of the positive eigenvalues; written to *n_eig_out (host).
+ * bb_kmeans_levels: exact one-dimensional k-means (dynamic programming over the sorted values: the global
+ *   minimum of the within-cluster sum of squares) of the positive eigenvalues, in the log domain if
+ *   log_domain != 0. intervals_out (host or device, n_levels x 2, ld ld_int >= n_levels): level 0 = highest
+ *   energy; edges at the midpoints between adjacent centroids (mapped back from the log domain), lowest
+ *   edge 0, highest DBL_MAX. BB_EINVAL if fewer than n_levels positive values. */
+#define BB_MAX_ESTIMATE 4096
+int bb_estimate_n_eig(bb_ctx* ctx, const double* lambda, int n, double energy_fraction, int* n_eig_out);
+int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int log_domain,
+                     double* intervals_out, int ld_int);
+
 /* ---- peak probes (measurement support) --------------------------------
  * kind: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2), 2 = MUFU sin+cos, 3 = DFMA. Runs a register-only
  * loop on every SM and returns operations per second in *ops_per_s (FMA counted as 1 op per

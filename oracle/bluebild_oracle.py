@@ -18,6 +18,11 @@ Functions and the passage each follows:
 ``synth``            Alg. 2 + Alg. 1 line 9 (C++: oracle/synth.cpp).
 ``brute``            the literal definition, tiny inputs (C++: oracle/brute.cpp).
 ``collect``          Alg. 1 end to end.
+``estimate_n_eig``   PAPER.md:152: minimum number of leading eigenvalues holding a given fraction
+                     of the total (positive) energy.
+``kmeans_levels``    PAPER.md:164: k-means clustering of the eigenvalues into energy levels; in one
+                     dimension the global optimum is found by dynamic programming over the sorted
+                     values (readings in DESIGN.md Q16).
 ===================  ==========================================================================
 
 Library primitives used as steps: numpy.linalg.cholesky, numpy.linalg.eigh, numpy.linalg.solve,
@@ -125,6 +130,78 @@ def level_weights(lam, intervals, filt="lsq"):
     inside = (lam[None, :] >= intervals[:, :1]) & (lam[None, :] <= intervals[:, 1:])
     d = lam if filt == "lsq" else np.ones_like(lam)
     return np.where(inside, d[None, :], 0.0)
+
+
+# ---------------------------------------------------------------------------------- parameter estimation
+def estimate_n_eig(lam, fraction):
+    """Smallest m such that the m largest eigenvalues hold >= fraction of the sum of the positive ones."""
+    lam = np.sort(np.asarray(lam, dtype=np.float64))[::-1]
+    pos = np.where(lam > 0.0, lam, 0.0)
+    total = 0.0
+    for x in pos:
+        total = total + x
+    target = fraction * total
+    run = 0.0
+    for a, x in enumerate(pos):
+        run = run + x
+        if run >= target:
+            return a + 1
+    return len(pos)
+
+
+def kmeans_levels(lam, n_levels, log_domain=True):
+    """Exact 1-D k-means of the positive eigenvalues (optionally of their logarithms): minimise the
+    within-cluster sum of squares over all partitions of the sorted values into n_levels contiguous
+    groups (optimal k-means clusters in one dimension are contiguous). Returns intervals
+    (n_levels, 2), level 0 = highest energy: edges at the midpoints between adjacent centroids
+    (mapped back from the log domain), lowest edge 0, highest the largest finite double."""
+    lam = np.asarray(lam, dtype=np.float64)
+    x = np.sort(np.log(lam[lam > 0.0]) if log_domain else lam[lam > 0.0])
+    n, k = len(x), int(n_levels)
+    if n < k:
+        raise ValueError("fewer positive eigenvalues than levels")
+    p1 = np.zeros(n + 1)
+    p2 = np.zeros(n + 1)
+    for i in range(n):
+        p1[i + 1] = p1[i] + x[i]
+        p2[i + 1] = p2[i] + x[i] * x[i]
+
+    def cost(i, j):                                         # sum of squared deviations of x[i:j]; i may be an array
+        s1 = p1[j] - p1[i]
+        s2 = p2[j] - p2[i]
+        return s2 - (s1 * s1) / (j - i)
+
+    big = np.finfo(np.float64).max
+    prev = np.full(n + 1, big)
+    for j in range(1, n + 1):
+        prev[j] = cost(0, j)
+    arg = np.zeros((k, n + 1), dtype=np.int64)
+    for c in range(1, k):
+        cur = np.full(n + 1, big)
+        for j in range(c + 1, n + 1):
+            i = np.arange(c, j)
+            v = prev[c:j] + cost(i, j)
+            b = int(np.argmin(v))                           # first minimum: the earliest split
+            cur[j] = v[b]
+            arg[c, j] = c + b
+        prev = cur
+    start = [0] * (k + 1)
+    start[k] = n
+    for c in range(k - 1, 0, -1):
+        start[c] = int(arg[c, start[c + 1]])
+    cen = [(p1[start[c + 1]] - p1[start[c]]) / (start[c + 1] - start[c]) for c in range(k)]
+    iv = np.zeros((k, 2))
+    for l in range(k):
+        c = k - 1 - l
+        lo, hi = 0.0, big
+        if c > 0:
+            e = 0.5 * (cen[c - 1] + cen[c])
+            lo = np.exp(e) if log_domain else e
+        if c < k - 1:
+            e = 0.5 * (cen[c] + cen[c + 1])
+            hi = np.exp(e) if log_domain else e
+        iv[l] = (lo, hi)
+    return iv
 
 
 # ---------------------------------------------------------------------------------- synthesis

@@ -26,7 +26,7 @@ _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_F
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
-           "bb_synth_launches", "bb_eig", "bb_probe_peak", "bb_status_string", "bb_version"]
+           "bb_synth_launches", "bb_eig", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_probe_peak", "bb_status_string", "bb_version"]
 
 _lib = None
 
@@ -64,6 +64,8 @@ def load_library(path: str = LIB_PATH):
         "bb_synth_timings": ([vp, pd, pd, pd, pd], i32),
         "bb_synth_launches": ([vp], i64),
         "bb_eig": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, vp, i32], i32),
+        "bb_estimate_n_eig": ([vp, vp, i32, f64, ctypes.POINTER(ctypes.c_int)], i32),
+        "bb_kmeans_levels": ([vp, vp, i32, i32, i32, vp, i32], i32),
         "bb_probe_peak": ([vp, i32, pd, pd], i32),
         "bb_status_string": ([i32], ctypes.c_char_p),
         "bb_version": ([], ctypes.c_char_p),
@@ -134,6 +136,22 @@ class Context:
             self._h = None
 
     __del__ = close
+
+    def estimate_n_eig(self, lam, energy_fraction: float) -> int:
+        """number of leading eigenvalues holding `energy_fraction` of the total energy."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        out = ctypes.c_int()
+        _check(_lib.bb_estimate_n_eig(self._h, lam.ctypes.data, lam.size, float(energy_fraction), ctypes.byref(out)),
+               "bb_estimate_n_eig")
+        return out.value
+
+    def kmeans_levels(self, lam, n_levels: int, log_domain: bool = True):
+        """level intervals (n_levels, 2) from exact 1-D k-means of the eigenvalues."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        iv = np.zeros((n_levels, 2), dtype=np.float64, order="F")
+        _check(_lib.bb_kmeans_levels(self._h, lam.ctypes.data, lam.size, int(n_levels), int(bool(log_domain)),
+                                     iv.ctypes.data, n_levels), "bb_kmeans_levels")
+        return iv
 
     def probe_peak(self, kind: int):
         ops, ms = ctypes.c_double(), ctypes.c_double()

@@ -478,3 +478,62 @@ extern "C" int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wave
   cudaGetLastError();
   return rc;
 }
+
+// ------------------------------------------------------------------------------ parameter estimation
+static int lambda_to_device(const double* lambda, int n, double** dev, bool* owned) {
+  *owned = false;
+  if (is_device_ptr(lambda)) { *dev = const_cast<double*>(lambda); return BB_OK; }
+  if (cudaMalloc(dev, (size_t)n * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+  *owned = true;
+  BB_CUDA(cudaMemcpy(*dev, lambda, (size_t)n * sizeof(double), cudaMemcpyHostToDevice));
+  return BB_OK;
+}
+
+extern "C" int bb_estimate_n_eig(bb_ctx* ctx, const double* lambda, int n, double energy_fraction, int* n_eig_out) {
+  if (!ctx || !lambda || !n_eig_out || n < 1 || n > BB_MAX_ESTIMATE || !(energy_fraction > 0.0) || energy_fraction > 1.0)
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(ctx->device));
+  double* lam = nullptr; bool owned = false; int* out = nullptr;
+  int rc = lambda_to_device(lambda, n, &lam, &owned);
+  if (rc == BB_OK && cudaMalloc(&out, sizeof(int)) != cudaSuccess) rc = BB_EALLOC;
+  if (rc == BB_OK) rc = bb_estimate_n_eig_dev(lam, n, energy_fraction, out, ctx->stream);
+  if (rc == BB_OK) {
+    cudaError_t e = cudaMemcpyAsync(n_eig_out, out, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { bb_note_cuda_error(e, "bb_estimate_n_eig", __FILE__, __LINE__); rc = BB_ECUDA; }
+  }
+  if (owned) cudaFree(lam);
+  cudaFree(out);
+  cudaGetLastError();
+  return rc;
+}
+
+extern "C" int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int log_domain,
+                                double* intervals_out, int ld_int) {
+  if (!ctx || !lambda || !intervals_out || n < 1 || n > BB_MAX_ESTIMATE || n_levels < 1 || n_levels > BB_MAX_LEVELS ||
+      n_levels > n || ld_int < n_levels)
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(ctx->device));
+  double* lam = nullptr; bool owned = false;
+  double* ws = nullptr; int* arg = nullptr; double* iv = nullptr; int* status = nullptr;
+  int rc = lambda_to_device(lambda, n, &lam, &owned);
+  if (rc == BB_OK && (cudaMalloc(&ws, bb_kmeans_workspace_doubles(n) * sizeof(double)) != cudaSuccess ||
+                      cudaMalloc(&arg, bb_kmeans_workspace_ints(n, n_levels) * sizeof(int)) != cudaSuccess ||
+                      cudaMalloc(&iv, (size_t)2 * n_levels * sizeof(double)) != cudaSuccess ||
+                      cudaMalloc(&status, sizeof(int)) != cudaSuccess)) rc = BB_EALLOC;
+  if (rc == BB_OK) rc = bb_kmeans_levels_dev(lam, n, n_levels, log_domain != 0, ws, arg, iv, n_levels, status, ctx->stream);
+  if (rc == BB_OK) {
+    int st_host = -1;
+    cudaError_t e = cudaMemcpyAsync(&st_host, status, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess && st_host == 0)
+      e = cudaMemcpy2D(intervals_out, (size_t)ld_int * sizeof(double), iv, (size_t)n_levels * sizeof(double),
+                       (size_t)n_levels * sizeof(double), 2, cudaMemcpyDefault);
+    if (e != cudaSuccess) { bb_note_cuda_error(e, "bb_kmeans_levels", __FILE__, __LINE__); rc = BB_ECUDA; }
+    else if (st_host != 0) rc = BB_EINVAL;                 // fewer positive eigenvalues than levels
+  }
+  if (owned) cudaFree(lam);
+  cudaFree(ws); cudaFree(arg); cudaFree(iv); cudaFree(status);
+  cudaGetLastError();
+  return rc;
+}

@@ -97,4 +97,11 @@ struct FilterList { int n; int kind[BB_MAX_FILTERS]; };
 int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int,
                             int n_intervals, FilterList filters, float* D_dev, int ldd, cudaStream_t st);
 
+// parameter estimation (estimate.cu); all pointers are device pointers
+int bb_estimate_n_eig_dev(const double* lam_dev, int n, double fraction, int* out_dev, cudaStream_t st);
+size_t bb_kmeans_workspace_doubles(int n);
+size_t bb_kmeans_workspace_ints(int n, int k);
+int bb_kmeans_levels_dev(const double* lam_dev, int n, int k, int log_domain, double* ws, int* arg, double* iv_dev, int ld_int,
+                         int* status_dev, cudaStream_t st);
+
 int bb_probe_run(int kind, int sm_count, cudaStream_t st, double* ops_per_s, double* ms);

@@ -192,3 +192,28 @@ def test_interference_probe(bb, ctx):
     assert min(dfma_alone, dfma_mma, imad_alone, imad_mma) > 0
     assert dfma_mma < 0.8 * dfma_alone, (dfma_alone, dfma_mma)
     assert imad_mma > 0.8 * imad_alone, (imad_alone, imad_mma)
+
+
+def test_parameter_estimation_matches_oracle(bb, ctx, oracle):
+    """bb_estimate_n_eig / bb_kmeans_levels (device glue) against the oracle: the counts must be
+    equal, the level edges equal to rounding (same fp64 expression on both sides)."""
+    from paper_2310_09200_b200 import workloads
+    w = workloads.make_workload(3)
+    lam_all = []
+    for n in (0, w.mid_collect(), w.cfg.n_collects - 1):
+        ci = w.collect_inputs(n)
+        lam, _ = ctx.eig(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], 512, want_B=False)
+        lam_all.append(lam)
+    lam_all = np.concatenate(lam_all)                       # 1536 eigenvalues pooled from three epochs
+    for frac in (0.5, 0.9, 0.99, 1.0):
+        assert ctx.estimate_n_eig(lam_all[:512], frac) == oracle.estimate_n_eig(lam_all[:512], frac)
+    for logd in (True, False):
+        for k in (1, 2, 4, 8):
+            got = ctx.kmeans_levels(lam_all, k, logd)
+            ref = oracle.kmeans_levels(lam_all, k, logd)
+            assert np.allclose(got, ref, rtol=1e-12, atol=0), (logd, k, got, ref)
+    rng = np.random.default_rng(3)
+    odd = np.concatenate([rng.lognormal(0, 3, 37), [-1.0, 0.0]])
+    assert np.allclose(ctx.kmeans_levels(odd, 5, True), oracle.kmeans_levels(odd, 5, True), rtol=1e-12)
+    with pytest.raises(bb.BluebildError):
+        ctx.kmeans_levels(np.array([1.0, -1.0, 0.0]), 2)

@@ -373,3 +373,46 @@ def test_filters_stack_as_interval_blocks(oracle):
     assert np.array_equal(both[2:], oracle.collect(S, None, xyz, wl, 6, iv, pix, filt="lsq"))
     D = oracle.level_weights(lam, iv, ("std", "lsq"))
     assert np.array_equal(D[2:], D[:2] * lam[None, :])
+
+
+# ---------------------------------------------------------------------------------- parameter estimation
+def test_estimate_n_eig_geometric_spectrum(oracle):
+    """lambda_a = 2^-a: the m leading values hold 1 - 2^-m of the (infinite) total, so 90 % needs m = 4 and
+    99.9 % needs m = 10; non-positive values carry no energy."""
+    lam = np.concatenate([2.0 ** -np.arange(1, 40), [-3.0, 0.0]])
+    rng = np.random.default_rng(5)
+    rng.shuffle(lam)
+    assert oracle.estimate_n_eig(lam, 0.9) == 4
+    assert oracle.estimate_n_eig(lam, 0.999) == 10
+    assert oracle.estimate_n_eig(lam, 1.0) <= 39
+
+
+@pytest.mark.parametrize("log_domain", [False, True])
+def test_kmeans_levels_is_the_global_optimum(oracle, log_domain):
+    """Brute force over ALL k^n assignments of 9 values to 3 clusters (not only contiguous ones): the dynamic
+    programme must reach the same minimum within-cluster sum of squares, and its edges must separate the
+    optimal clusters."""
+    import itertools
+    rng = np.random.default_rng(17 + log_domain)
+    lam = np.concatenate([rng.uniform(90, 110, 3), rng.uniform(9, 12, 3), rng.uniform(0.8, 1.3, 3)]) * rng.uniform(0.5, 2)
+    x = np.log(lam) if log_domain else lam
+    best, best_lab = np.inf, None
+    for lab in itertools.product(range(3), repeat=9):
+        lab = np.array(lab)
+        if len(set(lab)) < 3:
+            continue
+        sse = sum(np.sum((x[lab == c] - x[lab == c].mean()) ** 2) for c in range(3))
+        if sse < best:
+            best, best_lab = sse, lab
+    iv = oracle.kmeans_levels(lam, 3, log_domain)
+    got = np.array([[l for l in range(3) if iv[l, 0] <= v <= iv[l, 1]] for v in lam]).ravel()
+    assert got.size == 9                                            # every value in exactly one level
+    sse = sum(np.sum((x[got == l] - x[got == l].mean()) ** 2) for l in range(3))
+    assert abs(sse - best) <= 1e-12 * best
+    assert iv[0, 1] == np.finfo(np.float64).max and iv[2, 0] == 0.0 and iv[0, 0] == iv[1, 1] and iv[1, 0] == iv[2, 1]
+    assert lam[got == 0].min() > lam[got == 1].max() > lam[got == 2].max()     # level 0 = highest energy
+
+
+def test_kmeans_levels_needs_enough_positive_values(oracle):
+    with pytest.raises(ValueError):
+        oracle.kmeans_levels([1.0, -2.0, 0.0], 2)
