@@ -43,7 +43,8 @@ def random_case(seed, n_ant, n_eig, n_levels, n_pix, extent=3000.0, fov=0.25, si
 @pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("n_ant,n_eig,n_levels,n_pix", [
     (1, 1, 1, 1), (16, 8, 2, 1000), (37, 5, 3, 513), (50, 13, 4, 777), (33, 16, 1, 257), (70, 31, 5, 300),
-    (64, 33, 2, 129), (40, 64, 8, 255), (48, 65, 3, 200), (20, 130, 2, 150), (24, 7, 32, 100)])
+    (64, 33, 2, 129), (40, 64, 8, 255), (48, 65, 3, 200), (20, 130, 2, 150), (24, 7, 32, 100),
+    (40, 64, 32, 300)])      # most shared memory: 32 levels x 64 eigenpairs
 def test_shapes_ragged_and_padded(bb, ctx, oracle, variant, n_ant, n_eig, n_levels, n_pix):
     c = random_case(1000 + n_ant + n_eig, n_ant, n_eig, n_levels, n_pix, signed=True)
     ref = oracle.synth(c["B"], c["D"], c["xyz"], c["pix"], c["wavelength"])
