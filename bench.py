@@ -364,6 +364,17 @@ def run_ours(args):
                         "flops_per_launch": flops_per_launch, "avg_launch_ms": avg_launch_ms,
                         "peak_basis": ("148 SM x 128 FP32 lanes x 2 x 1.965 GHz (derived, DESIGN.md)" if bound == "alu" else
                                        ("1.0" if args.variant == "fp16x3" else "0.5") + " x measured bf16 burst (MEASURED_PEAKS.json); useful flops = 8/term, issued = 24/term")}
+    # DRAM traffic of one launch of this kernel, from the committed `ncu --set full` capture of the same command
+    prof = os.path.join(ROOT, "profiles", "r01_%s_ncu_full.csv" % args.variant)
+    if args.config == 4 and os.path.exists(prof):
+        try:
+            import csv
+            mb = {r[0]: float(r[2]) for r in csv.reader(open(prof)) if len(r) >= 3 and r[0].startswith("dram__bytes_") and r[1] == "Mbyte"}
+            if "dram__bytes_read.sum" in mb and "dram__bytes_write.sum" in mb:
+                line["roofline"]["traffic"] = (mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]) * 1e6
+                line["roofline"]["traffic_source"] = "profiles/" + os.path.basename(prof)
+        except Exception:
+            pass
     if bound == "tensor":
         # the split-precision scheme issues 3 tensor passes per useful one: 24 flops per term on the pipe
         line["roofline"]["issued_tflops"] = 3.0 * achieved_tflops
