@@ -96,6 +96,20 @@ int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig, double wa
                         int ldxyz, const double* intervals, int ld_int, int n_filters,
                         const int* filters, int gram_mode);
 
+/* ---- collect_batch: Algorithm 1 for n_collects time steps / channels in one call (the
+ * eigendecomposition is repeated for every time step and band). Same per-collect semantics as
+ * bb_synth_collect (one LSQ filter, sinc Gram), applied in order c = 0 .. n_collects-1; the Gram matrices,
+ * Cholesky factorisations and Hermitian eigensolves run as batched device calls (16 at a time).
+ *   wavelengths  n_collects float64, HOST pointer
+ *   S, xyz       collect c starts at S + c * stride_s, xyz + c * stride_xyz (strides in elements)
+ *   W            NULL (identity), or collect c at W + c * stride_w; stride_w == 0 shares one W
+ * If any Gram matrix is not positive definite or a solve fails, the collects of earlier groups stay
+ * accumulated and the call returns the error. Synchronises the context stream. */
+int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, int n_beam, int n_eig,
+                           const double* wavelengths, const bb_c32* W, int ldw, int64_t stride_w,
+                           const bb_c32* S, int lds, int64_t stride_s, const double* xyz, int ldxyz,
+                           int64_t stride_xyz, const double* intervals, int ld_int);
+
 /* ---- collect_eig: the hot path only (Algorithm 2 + Alg. 1 line 9, Eq. 15, 20) ---------------
  * I_l(r_j) += sum_k D[l,k] | sum_i conj(B_ik) exp(+j 2 pi <xyz_i, r_j> / wavelength) |^2
  *   B   n_ant x n_eig complex64 (= W V), ld ldb

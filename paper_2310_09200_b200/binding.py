@@ -25,7 +25,7 @@ GRAM_MODES = {"sinc": 0, "identity": 1}
 _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_FP16X3, 0: 0, 1: 1, 2: 2}
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
-           "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
+           "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_launches", "bb_eig", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_probe_peak", "bb_status_string", "bb_version"]
 
 _lib = None
@@ -58,6 +58,7 @@ def load_library(path: str = LIB_PATH):
         "bb_synth_reset": ([vp], i32),
         "bb_synth_collect": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32], i32),
         "bb_synth_collect_ex": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32, i32, vp, i32], i32),
+        "bb_synth_collect_batch": ([vp, i32, i32, i32, i32, vp, vp, i32, i64, vp, i32, i64, vp, i32, i64, vp, i32], i32),
         "bb_synth_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
         "bb_synth_flush": ([vp], i32),
         "bb_synth_get": ([vp, i32, vp], i32),
@@ -211,6 +212,28 @@ class StandardSynthesis:
         _check(_lib.bb_synth_collect_ex(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx,
                                         Ip, ldi, len(kinds), ctypes.cast(arr, ctypes.c_void_p), GRAM_MODES[gram]),
                "bb_synth_collect_ex")
+
+    def collect_batch(self, S, W, xyz, wavelengths, n_eig, intervals):
+        """Algorithm 1 for several collects with batched device eigensolves. S: (T, n_beam, n_beam) complex64,
+        xyz: (T, n_ant, 3) float64, W: None, (n_ant, n_beam) shared, or (T, n_ant, n_beam); numpy arrays."""
+        S = np.ascontiguousarray(np.transpose(np.asarray(S, dtype=np.complex64), (0, 2, 1)))      # column-major slices
+        X = np.ascontiguousarray(np.transpose(np.asarray(xyz, dtype=np.float64), (0, 2, 1)))
+        T, n_beam = S.shape[0], S.shape[1]
+        n_ant = X.shape[2]
+        wl = np.ascontiguousarray(np.broadcast_to(np.asarray(wavelengths, dtype=np.float64), (T,)))
+        Wp, ldw, sw = None, 0, 0
+        if W is not None:
+            W = np.asarray(W, dtype=np.complex64)
+            if W.ndim == 2:
+                W = np.ascontiguousarray(W.T)
+            else:
+                W = np.ascontiguousarray(np.transpose(W, (0, 2, 1)))
+                sw = n_ant * n_beam
+            Wp, ldw = W.ctypes.data, n_ant
+        keep = []
+        Ip, _, _, ldi = _marshal(intervals, np.float64, keep)
+        _check(_lib.bb_synth_collect_batch(self._h, T, n_ant, n_beam, int(n_eig), wl.ctypes.data, Wp, ldw, sw, S.ctypes.data, n_beam,
+                                           n_beam * n_beam, X.ctypes.data, n_ant, 3 * n_ant, Ip, ldi), "bb_synth_collect_batch")
 
     def collect_eig(self, B, D, xyz, wavelength):
         keep = []

@@ -406,6 +406,85 @@ extern "C" int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig
   return enqueue_prepared(s, n_ant, n_eig, wavelength, Bd, n_ant, Dd, s->n_levels, Xd, ldx2);
 }
 
+// Algorithm 1 for n_collects time steps / channels at once: the eigenproblems are solved as one batch.
+extern "C" int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, int n_beam, int n_eig, const double* wavelengths,
+                                      const bb_c32* W, int ldw, int64_t stride_w, const bb_c32* S, int lds, int64_t stride_s,
+                                      const double* xyz, int ldxyz, int64_t stride_xyz, const double* intervals, int ld_int) {
+  if (!s || !S || !xyz || !intervals || !wavelengths || n_collects < 1 || n_ant < 1 || n_beam < 1 || n_eig < 1 || n_eig > n_beam ||
+      n_beam > BB_MAX_BEAMS || lds < n_beam || ldxyz < n_ant || ld_int < s->n_levels || (W && ldw < n_ant) ||
+      (!W && n_beam != n_ant) || n_ant > (1 << 20) || stride_s < (int64_t)lds * n_beam || stride_xyz < (int64_t)ldxyz * 3 ||
+      (W && stride_w != 0 && stride_w < (int64_t)ldw * n_beam) || is_device_ptr(wavelengths))
+    return BB_EINVAL;
+  for (int c = 0; c < n_collects; ++c)
+    if (!(wavelengths[c] > 0.0)) return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(s->ctx->device));
+  int rc = ensure_queue(s, n_ant, n_beam, n_eig);
+  if (rc != BB_OK) return rc;
+  if (!s->ctx->glue && (rc = bb_glue_create(&s->ctx->glue)) != BB_OK) return rc;
+  cudaStream_t st = s->ctx->stream;
+  const int L = s->n_levels;
+  // device mirrors of host inputs (synchronous copies: this is glue) and per-batch outputs
+  std::vector<void*> tmp;
+  auto dev_copy = [&](const void* p, size_t bytes) -> const void* {
+    if (!p || is_device_ptr(p)) return p;
+    void* d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    tmp.push_back(d);
+    if (cudaMemcpy(d, p, bytes, cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return d;
+  };
+  auto dev_alloc = [&](size_t bytes) -> void* {
+    void* d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    tmp.push_back(d);
+    return d;
+  };
+  const size_t nS = (size_t)(n_collects - 1) * stride_s + (size_t)lds * n_beam;
+  const size_t nX = (size_t)(n_collects - 1) * stride_xyz + (size_t)ldxyz * 3;
+  const size_t nW = W ? (size_t)(stride_w ? n_collects - 1 : 0) * stride_w + (size_t)ldw * n_beam : 0;
+  const bb_c32* Sd = (const bb_c32*)dev_copy(S, nS * sizeof(bb_c32));
+  const double* Xd = (const double*)dev_copy(xyz, nX * sizeof(double));
+  const bb_c32* Wd = W ? (const bb_c32*)dev_copy(W, nW * sizeof(bb_c32)) : nullptr;
+  const double* wl_d = (const double*)dev_copy(wavelengths, (size_t)n_collects * sizeof(double));
+  double* iv_d = (double*)dev_alloc((size_t)2 * L * sizeof(double));
+  double* lam_d = (double*)dev_alloc((size_t)n_collects * n_eig * sizeof(double));
+  bb_c32* B_d = (bb_c32*)dev_alloc((size_t)n_collects * n_ant * n_eig * sizeof(bb_c32));
+  float* D_d = (float*)dev_alloc((size_t)n_collects * L * n_eig * sizeof(float));
+  rc = BB_OK;
+  if (!Sd || !Xd || (W && !Wd) || !wl_d || !iv_d || !lam_d || !B_d || !D_d) rc = BB_EALLOC;
+  if (rc == BB_OK && cudaMemcpy2D(iv_d, (size_t)L * sizeof(double), intervals, (size_t)ld_int * sizeof(double), (size_t)L * sizeof(double),
+                                  2, cudaMemcpyDefault) != cudaSuccess) { cudaGetLastError(); rc = BB_ECUDA; }
+  FilterList fl{};
+  fl.n = 1; fl.kind[0] = BB_FILTER_LSQ;
+  const int group = 16;                                    // eigenproblems per batched solve (bounded workspace)
+  for (int c0 = 0; rc == BB_OK && c0 < n_collects; c0 += group) {
+    const int nb = n_collects - c0 < group ? n_collects - c0 : group;
+    cudaEvent_t e0 = get_event(s), e1 = get_event(s), e2 = get_event(s), e3 = get_event(s);
+    rc = bb_glue_eig_batch(s->ctx->glue, st, nb, n_ant, n_beam, n_eig, wl_d + c0, Wd ? Wd + (size_t)c0 * stride_w : nullptr, ldw,
+                           stride_w, Sd + (size_t)c0 * stride_s, lds, stride_s, Xd + (size_t)c0 * stride_xyz, ldxyz, stride_xyz,
+                           lam_d + (size_t)c0 * n_eig, B_d + (size_t)c0 * n_ant * n_eig, e0, e1, e2, e3);
+    if (rc != BB_OK) {
+      s->free_ev.push_back(e0); s->free_ev.push_back(e1); s->free_ev.push_back(e2); s->free_ev.push_back(e3);
+      break;
+    }
+    s->spans.push_back(Span{e0, e1, T_GRAM});
+    s->spans.push_back(Span{e2, e3, T_EIG});
+    s->launches += 10;                                     // this file's batched kernels (library calls not counted)
+    for (int c = c0; rc == BB_OK && c < c0 + nb; ++c) {
+      float* Dc = D_d + (size_t)c * L * n_eig;
+      rc = bb_launch_level_weights(lam_d + (size_t)c * n_eig, n_eig, iv_d, L, L, fl, Dc, L, st);
+      if (rc != BB_OK) break;
+      s->launches += 1;
+      rc = enqueue_prepared(s, n_ant, n_eig, wavelengths[c], B_d + (size_t)c * n_ant * n_eig, n_ant, Dc, L,
+                            Xd + (size_t)c * stride_xyz, ldxyz);
+    }
+  }
+  cudaStreamSynchronize(st);                               // the prep kernels have consumed the temporaries
+  for (void* d : tmp) cudaFree(d);
+  cudaGetLastError();
+  return rc;
+}
+
 extern "C" int bb_synth_get(bb_synth* s, int level, float* out) {
   if (!s || !out || level < 0 || level >= s->n_levels) return BB_EINVAL;
   BB_CUDA(cudaSetDevice(s->ctx->device));

@@ -92,6 +92,10 @@ int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, 
                 const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
                 double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
                 cudaEvent_t ev_eig0, cudaEvent_t ev_eig1, int gram_mode = BB_GRAM_SINC);
+int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, int nb, int n_ant, int n_beam, int n_eig, const double* wavelength_dev,
+                      const bb_c32* W, int ldw, int64_t stride_w, const bb_c32* S, int lds, int64_t stride_s, const double* xyz,
+                      int ldxyz, int64_t stride_xyz, double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
+                      cudaEvent_t ev_eig0, cudaEvent_t ev_eig1);
 struct FilterList { int n; int kind[BB_MAX_FILTERS]; };
 // D[f * n_intervals + i, k] = d_f(lambda_k) [min_i <= lambda_k <= max_i]
 int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int,
