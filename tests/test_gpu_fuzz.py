@@ -1,0 +1,45 @@
+"""Randomised shapes through the C ABI: the three kernel variants must agree with each other and each must be
+bit-identical run to run (the mbarrier / TMEM pipelines have no data-dependent ordering). compute-sanitizer is not
+available on the GPU pool, so this and the edge tests are what exercises the ragged paths of the pipelines."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def test_random_shapes_agree_across_variants_and_runs():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2310_09200_b200 import binding
+    binding.load_library()
+    ctx = binding.Context(0)
+    rng = np.random.default_rng(20231009)
+    worst = 0.0
+    for case in range(120):
+        n_ant = int(rng.integers(1, 200)); n_eig = int(rng.integers(1, 140)); L = int(rng.integers(1, 12))
+        n_pix = int(rng.integers(1, 3000)); n_col = int(rng.integers(1, 40))
+        fov = rng.uniform(0.01, 0.6); ext = 10 ** rng.uniform(1, 4.5); wl = rng.uniform(0.5, 10)
+        lm = rng.uniform(-fov, fov, size=(n_pix, 2))
+        pix = np.asfortranarray(np.column_stack([lm, np.sqrt(1 - np.sum(lm * lm, axis=1))]))
+        items = []
+        for _ in range(n_col):
+            B = ((rng.normal(size=(n_ant, n_eig)) + 1j * rng.normal(size=(n_ant, n_eig))) * 10 ** rng.uniform(-3, 2))
+            D = rng.uniform(0.1, 3, size=(L, n_eig)) * (rng.random((L, n_eig)) < 0.4)
+            items.append((np.asfortranarray(B.astype(np.complex64)), np.asfortranarray(D.astype(np.float32)),
+                          np.asfortranarray(rng.uniform(-ext, ext, size=(n_ant, 3)))))
+        imgs = {}
+        for variant in ("fp32", "fp16x3", "fp16x3", "tf32x3", "tf32x3"):
+            s = binding.StandardSynthesis(ctx, pix, L, variant)
+            for B, D, xyz in items:
+                s.collect_eig(B, D, xyz, wl)
+            im = s.images()
+            if variant in imgs:
+                assert np.array_equal(imgs[variant], im), ("not bit-identical run to run", variant, n_ant, n_eig, L, n_pix, n_col)
+            imgs[variant] = im
+        ref = imgs["fp32"].astype(np.float64)
+        peak = np.max(np.abs(ref)) or 1.0
+        for v in ("fp16x3", "tf32x3"):
+            err = np.max(np.abs(imgs[v] - ref)) / peak
+            worst = max(worst, err)
+            assert err < 5e-5, (v, err, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
+    print("worst max-abs / peak between variants: %.2e" % worst)
