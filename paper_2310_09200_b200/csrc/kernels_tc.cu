@@ -20,8 +20,11 @@
 //     p'_d = IH_d 2^-8 + PL_d      (IH = rint(p' 2^8) int32, |PL| <= 2^-9; per antenna, written by prep)
 //     r'_d = JH_d 2^-24 + RL_d     (JH = rint(r' 2^24) int32, |RL| <= 2^-25; per pixel, once per thread)
 //     frac(<p', r'>) = [ sum_d IH_d * JH_d mod 2^32 ] 2^-32  +  sum_d ( PH_d RL_d + PL_d r'_d )      (turns)
-//   three wrapping 32-bit IMADs give the large part exactly; the small part (< 2^-6 turns) is 6 fp32 FMAs.
-//   The 32-bit fraction is converted with the 1.5*2^23 magic-add (no I2F on the MUFU pipe), then MUFU.SIN/COS.
+//   three wrapping 32-bit IMADs give the large part exactly; the small part (< 2^-6 turns) is bilinear of rank 6:
+//   TF32 mode evaluates it with 6 fp32 FMAs per (antenna, pixel); FP16 mode runs it as a K = 16 mini-GEMM on the
+//   tensor core (pixels x 16 antennas per chunk, hi/lo of both sides folded into K) whose result lands in the
+//   lo half of the A stage the producers fill next. The 32-bit fraction becomes a float by an integer add onto
+//   an exponent pattern (no I2F on the MUFU pipe), then one FFMA and MUFU.SIN/COS.
 //
 // CTA = 2 pixel tiles of 128 (256 pixels), 608 threads, 1 CTA per SM, all 512 TMEM columns:
 //   warps 0-15 producers + epilogue (two groups alternating chunks): phase generator, hi/lo split,
