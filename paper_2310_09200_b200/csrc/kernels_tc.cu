@@ -214,8 +214,10 @@ __device__ __forceinline__ void phase_cs_ls(const int4& ih, float lsm, int jx, i
   c = __cosf(x);
   s = __sinf(x);
 }
+// hi = x rounded to nearest at TF32's 10-bit mantissa (add half an ulp, then clear the 13 low bits), lo = x - hi exactly;
+// the tensor core truncates lo to TF32 itself (error 2^-11 of a 2^-11 term).
 __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
-  hi = __float_as_uint(x) & 0xFFFFE000u;
+  hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
   lo = __float_as_uint(x - __uint_as_float(hi));
 }
 // (cos, sin) -> packed FP16 pairs: hi = rn16(x), lo = rn16(x - hi); K order (cos, sin) = (low, high) half.
