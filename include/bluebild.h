@@ -6,14 +6,24 @@
  *
  * Conventions for EVERY entry point
  *   - Every data pointer may be a HOST or a DEVICE pointer (classified with
- *     cudaPointerGetAttributes). Host buffers are snapshotted before the call returns; device
- *     buffers are read in stream order on the context stream and must stay valid until work
- *     already enqueued on that stream has consumed them (i.e. until bb_synth_flush/get returns
- *     or the stream is synchronised).
+ *     cudaPointerGetAttributes). Host buffers are snapshotted before the call returns. Device
+ *     buffers are read in stream order with respect to the context stream: after all work that
+ *     was enqueued on it when the call was made, and the context stream is made to wait for the
+ *     kernel or copy that consumes them — so they may be overwritten or freed by later work on
+ *     that stream, but not from the host or another stream before the context stream (or a later
+ *     synchronising call: bb_synth_get / _status / _timings / _reset) has been synchronised.
+ *     bb_synth_flush alone does NOT synchronise.
+ *   - Work runs on streams the context owns (glue and synthesizer overlap); the
+ *     context stream carries the ordering, also for results: after bb_synth_flush it waits for
+ *     the synthesizer, so later work on it sees the images.
  *   - The caller owns all buffers; the library never frees or retains caller memory.
  *   - Return value: BB_OK or an error code; no exception crosses the ABI. All arguments are
  *     validated before any launch, so a failed call leaves the level images unchanged and the
- *     handle usable.
+ *     handle usable. Conditions only the device can see (Gram matrix not positive definite,
+ *     eigensolver failure, antenna coordinates beyond the phase generator's range) do not stop
+ *     the call: the offending collect contributes NOTHING to the images and a sticky flag is
+ *     raised, which the next bb_synth_get / bb_synth_status returns as BB_ENOTPOSDEF /
+ *     BB_ENOCONV / BB_EUNSUPPORTED (cleared by bb_synth_reset).
  *   - All matrices are column-major with an explicit leading dimension (in elements).
  *   - Complex single precision is interleaved (re, im) pairs of float (bb_c32).
  *   - There is no CPU fallback: without a CUDA device bb_ctx_create fails with BB_ECUDA.
@@ -53,7 +63,7 @@ enum {
  * device: CUDA ordinal. cuda_stream: a cudaStream_t (may be NULL = default stream) on which all
  * work of handles created from this context is enqueued. */
 int bb_ctx_create(int device, void* cuda_stream, bb_ctx** out);
-int bb_ctx_destroy(bb_ctx* ctx);
+int bb_ctx_destroy(bb_ctx* ctx); /* BB_ESTATE while imaging handles created from it are alive */
 
 /* ---- imaging handle -----------------------------------------------------------------------
  * pix: X_pix of Table 1: n_pix x 3 pixel unit vectors, column-major with leading
@@ -76,7 +86,9 @@ int bb_synth_reset(bb_synth* s); /* drop pending collects and zero the level ima
  *   S   n_beam x n_beam complex64 Hermitian, full storage, ld lds (used as (S+S^H)/2)
  *   xyz n_ant x 3 float64 metres, ld ldxyz (P_icrs of Table 1)
  *   intervals n_levels x 2 float64, ld ld_int: column 0 = min, column 1 = max
- * Limits: 1 <= n_eig <= n_beam <= BB_MAX_BEAMS, n_ant >= 1, wavelength > 0. */
+ * Limits: 1 <= n_eig <= n_beam <= BB_MAX_BEAMS, n_ant >= 1, wavelength > 0; coordinate range as for
+ * bb_synth_collect_eig. The call stages its inputs; the glue runs batched over up to 32 staged collects
+ * (when 32 are staged, on bb_synth_flush, or on bb_synth_get) on the context's glue stream. */
 int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength,
                      const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz,
                      int ldxyz, const double* intervals, int ld_int);
@@ -99,12 +111,13 @@ int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig, double wa
 /* ---- collect_batch: Algorithm 1 for n_collects time steps / channels in one call (the
  * eigendecomposition is repeated for every time step and band). Same per-collect semantics as
  * bb_synth_collect (one LSQ filter, sinc Gram), applied in order c = 0 .. n_collects-1; the Gram matrices,
- * Cholesky factorisations and Hermitian eigensolves run as batched device calls (16 at a time).
+ * Cholesky factorisations and Hermitian eigensolves run as batched device calls (32 collects at a time); the
+ * synthesizer of one group runs while the glue of the next is in progress.
  *   wavelengths  n_collects float64, HOST pointer
  *   S, xyz       collect c starts at S + c * stride_s, xyz + c * stride_xyz (strides in elements)
  *   W            NULL (identity), or collect c at W + c * stride_w; stride_w == 0 shares one W
- * If any Gram matrix is not positive definite or a solve fails, the collects of earlier groups stay
- * accumulated and the call returns the error. Synchronises the context stream. */
+ * A collect whose Gram matrix is not positive definite or whose solve fails contributes nothing and raises the
+ * sticky flag (see the conventions above). Does not synchronise. */
 int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, int n_beam, int n_eig,
                            const double* wavelengths, const bb_c32* W, int ldw, int64_t stride_w,
                            const bb_c32* S, int lds, int64_t stride_s, const double* xyz, int ldxyz,
@@ -117,7 +130,11 @@ int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, int n_beam, i
  *   xyz n_ant x 3 float64, ld ldxyz
  * The call enqueues a small preparation kernel and queues the collect; the fused synthesizer
  * kernel runs when the queue is full, on bb_synth_flush, or on bb_synth_get, looping over all
- * queued collects inside one launch (every time step and band). */
+ * queued collects inside one launch (every time step and band).
+ * Coordinate range of the phase generator, with p' = (xyz - mean(xyz)) / wavelength and r' the pixel vectors
+ * minus the centre of their bounding box: FP32 variant |p'| max|r'| < 2^19 turns; tensor variants
+ * |p'_x|, |p'_y|, |p'_z| < 2^23 wavelengths. Checked on the device: a collect beyond it contributes nothing
+ * and bb_synth_get / bb_synth_status return BB_EUNSUPPORTED. */
 int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wavelength, const bb_c32* B,
                          int ldb, const float* D, int ldd, const double* xyz, int ldxyz);
 
@@ -125,9 +142,13 @@ int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wavelength, c
 int bb_synth_flush(bb_synth* s);
 
 /* Copy level image `level` (n_pix float32, pixel order of pix) to out (host or device).
- * Flushes pending collects and synchronises the context stream. Images are plain sums over
- * collects (Alg. 1 line 9: "+="; no division by the number of collects). */
+ * Flushes pending collects and synchronises. Images are plain sums over collects (Alg. 1 line 9:
+ * "+="; no division by the number of collects). The image is copied even when the return value
+ * reports a sticky device-side condition (it then holds the sum of the collects that were fine). */
 int bb_synth_get(bb_synth* s, int level, float* out);
+
+/* Flush, synchronise and return the sticky device-side condition of the handle (BB_OK if none). */
+int bb_synth_status(bb_synth* s);
 
 /* Device-measured times (CUDA events, ms) accumulated since create/reset; any may be NULL. */
 int bb_synth_timings(bb_synth* s, double* gram_ms, double* eig_ms, double* prep_ms, double* synth_ms);
@@ -141,6 +162,15 @@ int64_t bb_synth_launches(bb_synth* s);
 int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W,
            int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz, double* lambda_out,
            bb_c32* B_out, int ldb_out);
+
+/* ---- level weights alone (Alg. 1 lines 7-8; filters PAPER.md:166) ----------------------
+ * D_out[f * n_intervals + i, k] = d_f(lambda_k) if intervals[i,0] <= lambda_k <= intervals[i,1] else 0, with
+ * d = lambda_k for BB_FILTER_LSQ and 1 for BB_FILTER_STD — the D that bb_synth_collect_eig takes, computed by the
+ * same kernel bb_synth_collect uses. lambda: n_eig float64; intervals: n_intervals x 2, ld ld_int; filters:
+ * n_filters entries, HOST pointer; D_out: (n_intervals * n_filters) x n_eig float32, ld ldd. Host or device
+ * pointers; synchronises the context stream. */
+int bb_level_weights(bb_ctx* ctx, const double* lambda, int n_eig, const double* intervals, int ld_int,
+                     int n_intervals, int n_filters, const int* filters, float* D_out, int ldd);
 
 /* ---- parameter estimation (Table 4 caption :593), device-side glue -------------
  * lambda: n (1..BB_MAX_ESTIMATE) eigenvalues in any order, host or device (one collect's, or pooled from a
@@ -156,15 +186,6 @@ int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, con
 int bb_estimate_n_eig(bb_ctx* ctx, const double* lambda, int n, double energy_fraction, int* n_eig_out);
 int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int log_domain,
                      double* intervals_out, int ld_int);
-
-/* ---- peak probes (measurement support) --------------------------------
- * kind: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2), 2 = MUFU sin+cos, 3 = DFMA. Runs a register-only
- * loop on every SM and returns operations per second in *ops_per_s (FMA counted as 1 op per
- * lane; kind 1 counts 2 per lane-instruction) and the kernel time in *ms.
- * kind 4/5 = DFMA chains on 8 warps per SM without / with a concurrent tcgen05.mma stream on the
- * same SM, kind 6/7 = the same for IMAD: *ms is the slowest warp's clock64 span at the nominal
- * maximum clock, *ops_per_s the lane-operations over that span (interference probe). */
-int bb_probe_peak(bb_ctx* ctx, int kind, double* ops_per_s, double* ms);
 
 const char* bb_status_string(int status);
 const char* bb_version(void);

@@ -26,7 +26,7 @@ _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_F
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
-           "bb_synth_launches", "bb_eig", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_probe_peak", "bb_status_string", "bb_version"]
+           "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version"]
 
 _lib = None
 
@@ -67,7 +67,8 @@ def load_library(path: str = LIB_PATH):
         "bb_eig": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, vp, i32], i32),
         "bb_estimate_n_eig": ([vp, vp, i32, f64, ctypes.POINTER(ctypes.c_int)], i32),
         "bb_kmeans_levels": ([vp, vp, i32, i32, i32, vp, i32], i32),
-        "bb_probe_peak": ([vp, i32, pd, pd], i32),
+        "bb_synth_status": ([vp], i32),
+        "bb_level_weights": ([vp, vp, i32, vp, i32, i32, i32, vp, vp, i32], i32),
         "bb_status_string": ([i32], ctypes.c_char_p),
         "bb_version": ([], ctypes.c_char_p),
     }
@@ -130,9 +131,16 @@ class Context:
             sp = ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
         _check(lib.bb_ctx_create(int(device), sp, ctypes.byref(h)), "bb_ctx_create")
         self._h, self._stream, self.device = h, stream, device
+        self._children = []                      # weak references to the imaging handles created from this context
 
     def close(self):
+        """Destroys the context; imaging handles created from it are closed first (bb_ctx_destroy refuses while any is alive)."""
         if getattr(self, "_h", None):
+            for ref in self._children:
+                child = ref()
+                if child is not None:
+                    child.close()
+            self._children = []
             _lib.bb_ctx_destroy(self._h)
             self._h = None
 
@@ -154,10 +162,17 @@ class Context:
                                      iv.ctypes.data, n_levels), "bb_kmeans_levels")
         return iv
 
-    def probe_peak(self, kind: int):
-        ops, ms = ctypes.c_double(), ctypes.c_double()
-        _check(_lib.bb_probe_peak(self._h, kind, ctypes.byref(ops), ctypes.byref(ms)), "bb_probe_peak")
-        return ops.value, ms.value
+    def level_weights(self, lam, intervals, filters=None):
+        """Alg. 1 l.7-8: D (n_levels, n_eig) float32 from eigenvalues and closed intervals (the library's own kernel)."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        iv = np.asfortranarray(np.asarray(intervals, dtype=np.float64).reshape(-1, 2))
+        kinds = [FILTERS[f] for f in (filters or ["lsq"])]
+        arr = (ctypes.c_int * len(kinds))(*kinds)
+        L = iv.shape[0] * len(kinds)
+        D = np.zeros((L, lam.size), dtype=np.float32, order="F")
+        _check(_lib.bb_level_weights(self._h, lam.ctypes.data, lam.size, iv.ctypes.data, iv.shape[0], iv.shape[0], len(kinds),
+                                     ctypes.cast(arr, ctypes.c_void_p), D.ctypes.data, L), "bb_level_weights")
+        return D
 
     def eig(self, S, W, xyz, wavelength, n_eig, want_B=True):
         """Alg. 1 lines 2-4: (lambda desc float64 (n_eig,), B complex64 (n_ant, n_eig))."""
@@ -183,9 +198,11 @@ class StandardSynthesis:
         _check(_lib.bb_synth_create(ctx._h, n_pix, Pp, ld, int(n_levels), _VARIANTS[variant], ctypes.byref(h)),
                "bb_synth_create")
         self._h, self.ctx, self.n_pix, self.n_levels = h, ctx, n_pix, n_levels
+        import weakref
+        ctx._children.append(weakref.ref(self))
 
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and _lib is not None:
             _lib.bb_synth_destroy(self._h)
             self._h = None
 
@@ -245,6 +262,11 @@ class StandardSynthesis:
 
     def flush(self):
         _check(_lib.bb_synth_flush(self._h), "bb_synth_flush")
+
+    def status(self):
+        """Flush, synchronise and raise if a collect was dropped on the device (Gram not positive definite,
+        eigensolver failure, coordinates beyond the phase generator's range)."""
+        _check(_lib.bb_synth_status(self._h), "bb_synth_status")
 
     def get(self, level: int, out=None):
         """Level image as float32 (n_pix,). `out` may be a numpy array or a torch CUDA tensor."""

@@ -2,7 +2,7 @@
 // eigenvectors that account for a user-defined percentage of the total energy"; "Level partitions
 // can be automatically determined using k-means clustering on the eigenvalues"; Table 4 caption PAPER.md:593).
 // Both work on a list of eigenvalues (one collect's, or pooled from a subset of the data) and are glue, not the
-// hot path: one CTA, fp64, deterministic (sequential sums in the order the oracle uses).
+// hot path: one CTA, fp64, deterministic.
 //   n_eig   sort descending; total = sum of the positive eigenvalues; smallest m with sum_{a<=m} lambda_a >= f total.
 //   k-means in one dimension has an exact solution: optimal clusters are contiguous in sorted order, so dynamic
 //           programming over the split points minimises the within-cluster sum of squares globally (DESIGN.md
@@ -52,10 +52,11 @@ __global__ void __launch_bounds__(kEstThreads) n_eig_kernel(const double* __rest
   }
 }
 
-// sse of sorted values i..j-1 from prefix sums: S2 - S1^2 / cnt (no FMA contraction: the oracle evaluates the same expression)
+// within-cluster sum of squares of the sorted values i..j-1 from the prefix sums of the CENTRED values
+// (y = x - mean of all values, which keeps S2 - S1^2 / cnt well conditioned for tightly packed spectra)
 __device__ __forceinline__ double seg_cost(const double* p1, const double* p2, int i, int j) {
-  const double s1 = __dadd_rn(p1[j], -p1[i]), s2 = __dadd_rn(p2[j], -p2[i]);
-  return __dadd_rn(s2, -__ddiv_rn(__dmul_rn(s1, s1), (double)(j - i)));
+  const double s1 = p1[j] - p1[i], s2 = p2[j] - p2[i];
+  return fmax(fma(-s1, s1 / (double)(j - i), s2), 0.0);
 }
 
 // workspace (global): x[np], p1[np+1], p2[np+1], dp[2][np+1], arg[k][np+1]
@@ -64,6 +65,7 @@ __global__ void __launch_bounds__(kEstThreads) kmeans_kernel(const double* __res
                                                             int ld_int, int* __restrict__ status) {
   extern __shared__ double sh[];
   __shared__ int np_s;
+  __shared__ double mean_s;
   for (int i = threadIdx.x; i < m; i += blockDim.x) {
     const double x = i < n ? lam[i] : -1.0;
     sh[i] = x > 0.0 ? (log_domain ? log(x) : x) : DBL_MAX;  // non-positive values sort to the end and are dropped
@@ -85,8 +87,12 @@ __global__ void __launch_bounds__(kEstThreads) kmeans_kernel(const double* __res
   if (np < k) { if (threadIdx.x == 0) *status = 1; return; }
   for (int i = threadIdx.x; i < np; i += blockDim.x) x[i] = sh[i];
   if (threadIdx.x == 0) {
+    double mean = 0.0;
+    for (int i = 0; i < np; ++i) mean += sh[i];
+    mean /= (double)np;
     p1[0] = 0.0; p2[0] = 0.0;
-    for (int i = 0; i < np; ++i) { p1[i + 1] = __dadd_rn(p1[i], sh[i]); p2[i + 1] = __dadd_rn(p2[i], __dmul_rn(sh[i], sh[i])); }
+    for (int i = 0; i < np; ++i) { const double y = sh[i] - mean; p1[i + 1] = p1[i] + y; p2[i + 1] = fma(y, y, p2[i]); }
+    mean_s = mean;
   }
   __syncthreads();
   // dp[c][j] = min cost of splitting the first j values into c + 1 clusters; arg[c][j] = start of the last one
@@ -100,8 +106,8 @@ __global__ void __launch_bounds__(kEstThreads) kmeans_kernel(const double* __res
       int bi = c;
       if (j >= c + 1)
         for (int i = c; i < j; ++i) {                      // last cluster = values i..j-1, the first i in c clusters
-          const double v = __dadd_rn(prev[i], seg_cost(p1, p2, i, j));
-          if (v < best) { best = v; bi = i; }              // ties: the earliest split, as the oracle's argmin
+          const double v = prev[i] + seg_cost(p1, p2, i, j);
+          if (v < best) { best = v; bi = i; }              // equal costs: the earliest split (any of them is optimal)
         }
       cur[j] = best;
       arg[(size_t)c * (m + 1) + j] = bi;
@@ -116,13 +122,13 @@ __global__ void __launch_bounds__(kEstThreads) kmeans_kernel(const double* __res
     for (int c = k - 1; c >= 1; --c) start[c] = arg[(size_t)c * (m + 1) + start[c + 1]];
     start[0] = 0;
     double cen[BB_MAX_LEVELS];
-    for (int c = 0; c < k; ++c) cen[c] = __ddiv_rn(__dadd_rn(p1[start[c + 1]], -p1[start[c]]), (double)(start[c + 1] - start[c]));
+    for (int c = 0; c < k; ++c) cen[c] = mean_s + (p1[start[c + 1]] - p1[start[c]]) / (double)(start[c + 1] - start[c]);
     // level l = cluster k - 1 - l (level 0 = highest energy); interval = [lower edge, upper edge]
     for (int l = 0; l < k; ++l) {
       const int c = k - 1 - l;
       double lo = 0.0, hi = DBL_MAX;
-      if (c > 0) { const double e = __dmul_rn(0.5, __dadd_rn(cen[c - 1], cen[c])); lo = log_domain ? exp(e) : e; }
-      if (c < k - 1) { const double e = __dmul_rn(0.5, __dadd_rn(cen[c], cen[c + 1])); hi = log_domain ? exp(e) : e; }
+      if (c > 0) { const double e = 0.5 * (cen[c - 1] + cen[c]); lo = log_domain ? exp(e) : e; }
+      if (c < k - 1) { const double e = 0.5 * (cen[c] + cen[c + 1]); hi = log_domain ? exp(e) : e; }
       iv[l] = lo;
       iv[l + ld_int] = hi;
     }

@@ -60,9 +60,22 @@ struct PrepArgs {
   int n_ant, n_eig, n_levels;
   double wavelength;
   double rc[3];
+  double rmax;                        // upper bound of |r'| over the handle's pixels (range check of the phase generator)
   unsigned char* packed;              // device: collect buffer
   float* weights;                     // device: [level][n_eig_pad]
+  int* status;                        // device: sticky BB_FLAG_* word of the handle
 };
+
+// Sticky device-side verdicts of a handle (read back by bb_synth_get / bb_synth_status). A collect that raises one
+// contributes nothing to the images: its level weights are written as zeros.
+enum { BB_FLAG_RANGE = 1, BB_FLAG_NOTPOSDEF = 2, BB_FLAG_NOCONV = 4 };
+
+// Phase-generator range limits, checked by the prep kernels against the centred antenna positions p' (wavelengths):
+//   FP32 variant:  |<p', r'>| < 2^19 turns (the fixed-point fraction is read from an fp64 sum anchored at 1.5 * 2^20);
+//                  enforced as |p'|_2 * rmax < 2^19
+//   tensor variants: |p'_d| < 2^23 wavelengths (IH = rint(p' 2^8) must fit an int32)
+constexpr double kFp32PhaseLimit = 524288.0;
+constexpr double kTcCoordLimit = 8388608.0;
 
 int bb_launch_prep_fp32(const Fp32Plan& plan, const PrepArgs& a, cudaStream_t st);
 int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st);
@@ -78,28 +91,41 @@ struct SynthArgs {
 int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
 
-// pixel preparation: bounding-box centre r_c and r' = r - r_c (SoA fp64)
+// pixel preparation: bounding-box centre r_c, r' = r - r_c (SoA fp64) and rmax = half the box diagonal >= max |r'|
 int bb_pixels_prepare(const double* pix_dev, int64_t n_pix, int64_t ld_pix, double* rprime,
-                      int64_t pix_stride, double rc_out[3], cudaStream_t st);
+                      int64_t pix_stride, double rc_out[3], double* rmax_out, cudaStream_t st);
 
-// glue (Alg. 1 lines 2-4) — glue.cu
+// glue (Alg. 1 lines 2-4) — glue.cu; everything is batched over collects and asynchronous on the given stream
 struct GlueWork;
+struct SubspaceWork;
+enum { GB_PSI = 0, GB_G, GB_W, GB_T, GB_S, GB_LAM, GB_VSEL, GB_B, GB_PTRS, GB_WORK, GB_SUB0, GB_SUB1, GB_SUB2, GB_SUB3, GB_SUB4, GB_SUB5,
+       kGlueBuffers };
 int bb_glue_create(GlueWork** out);
 void bb_glue_destroy(GlueWork* g);
-// Computes lambda (n_eig, descending, device fp64) and B = W V (n_ant x n_eig complex64, device,
-// ld n_ant). W/S/xyz are device pointers. Timed with the given events (may be null).
-int bb_glue_eig(GlueWork* g, cudaStream_t st, int n_ant, int n_beam, int n_eig, double wavelength,
-                const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz,
-                double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
-                cudaEvent_t ev_eig0, cudaEvent_t ev_eig1, int gram_mode = BB_GRAM_SINC);
-int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, int nb, int n_ant, int n_beam, int n_eig, const double* wavelength_dev,
-                      const bb_c32* W, int ldw, int64_t stride_w, const bb_c32* S, int lds, int64_t stride_s, const double* xyz,
-                      int ldxyz, int64_t stride_xyz, double* lambda_dev, bb_c32* B_dev, cudaEvent_t ev_gram0, cudaEvent_t ev_gram1,
-                      cudaEvent_t ev_eig0, cudaEvent_t ev_eig1);
+int bb_glue_grow(GlueWork* g, int slot, size_t bytes, cudaStream_t st);   // scratch array `slot` of at least `bytes`
+void* bb_glue_buffer(GlueWork* g, int slot);
+struct GlueBatch {
+  int nb, n_ant, n_beam, n_eig, gram_mode;
+  const double* wavelength; int64_t stride_wl;       // device, one per collect
+  const bb_c32* W; int ldw; int64_t stride_w;        // device or NULL; stride_w == 0: one W for all collects
+  const bb_c32* S; int lds; int64_t stride_s;        // device
+  const double* xyz; int ldxyz; int64_t stride_xyz;  // device
+  double* lambda_dev; int64_t stride_lam;            // out: n_eig eigenvalues per collect, descending
+  bb_c32* B_dev; int64_t stride_b;                   // out: B = W V, n_ant x n_eig complex64, ld n_ant
+  int* info_dev;                                     // out: [2 nb] Cholesky verdicts, then eigensolver verdicts
+  cudaEvent_t ev_gram0, ev_gram1, ev_eig0, ev_eig1;  // may be null
+};
+int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, const GlueBatch& a, int* launches);
 struct FilterList { int n; int kind[BB_MAX_FILTERS]; };
-// D[f * n_intervals + i, k] = d_f(lambda_k) [min_i <= lambda_k <= max_i]
+// D[f * n_intervals + i, k] = d_f(lambda_k) [min_i <= lambda_k <= max_i]; zeros + status flag when *info_* != 0
 int bb_launch_level_weights(const double* lambda_dev, int n_eig, const double* intervals_dev, int ld_int,
-                            int n_intervals, FilterList filters, float* D_dev, int ldd, cudaStream_t st);
+                            int n_intervals, FilterList filters, float* D_dev, int ldd, const int* info_chol,
+                            const int* info_eig, int* status_dev, cudaStream_t st);
+
+// leading eigenpairs of nb Hermitian matrices by block subspace iteration (eig_subspace.cu). On return *used says
+// whether the fast path produced the result (vectors / values descending in *vecs / *lams) or the caller must run
+// the full eigensolve on C (left untouched in that case).
+void bb_subspace_destroy(SubspaceWork* w);
 
 // parameter estimation (estimate.cu); all pointers are device pointers
 int bb_estimate_n_eig_dev(const double* lam_dev, int n, double fraction, int* out_dev, cudaStream_t st);
@@ -107,5 +133,3 @@ size_t bb_kmeans_workspace_doubles(int n);
 size_t bb_kmeans_workspace_ints(int n, int k);
 int bb_kmeans_levels_dev(const double* lam_dev, int n, int k, int log_domain, double* ws, int* arg, double* iv_dev, int ld_int,
                          int* status_dev, cudaStream_t st);
-
-int bb_probe_run(int kind, int sm_count, cudaStream_t st, double* ops_per_s, double* ms);

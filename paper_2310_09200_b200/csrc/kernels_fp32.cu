@@ -20,12 +20,6 @@
 //     per launch (8*L bytes per pixel per launch).
 #include "internal.h"
 #include <cuda.h>
-#include <cstdio>
-#include <cstdlib>
-
-#ifndef BB_ORDER
-#define BB_ORDER 0
-#endif
 
 namespace {
 
@@ -162,7 +156,6 @@ synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_
         // a2: 4 FFMA2 per (pixel, eigen-pair). Order matters: an FFMA2 reads 5 registers (scalar, pair,
         // accumulator pair) and the register file delivers 2 per bank per FFMA2 slot, so consecutive
         // FFMA2 must share an operand through the operand-reuse cache.
-#if BB_ORDER == 0
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
           const float4 b = brow[(size_t)i * ROW4 + q];
@@ -176,26 +169,6 @@ synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_
 #pragma unroll
           for (int p = 0; p < PT; ++p) im[p][q] = __ffma2_rn(make_float2(cs[p], cs[p]), bi, im[p][q]);
         }
-#else
-        {
-          float4 b[NQ];
-#pragma unroll
-          for (int q = 0; q < NQ; ++q) b[q] = brow[(size_t)i * ROW4 + q];
-#pragma unroll
-          for (int p = 0; p < PT; ++p) {
-            const float2 cc = make_float2(cs[p], cs[p]), ss = make_float2(sn[p], sn[p]);
-            const float2 ns = make_float2(-sn[p], -sn[p]);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) re[p][q] = __ffma2_rn(cc, make_float2(b[q].x, b[q].y), re[p][q]);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) im[p][q] = __ffma2_rn(cc, make_float2(b[q].z, b[q].w), im[p][q]);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) re[p][q] = __ffma2_rn(ss, make_float2(b[q].z, b[q].w), re[p][q]);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) im[p][q] = __ffma2_rn(ns, make_float2(b[q].x, b[q].y), im[p][q]);
-          }
-        }
-#endif
 #pragma unroll
         for (int p = 0; p < PT; ++p) { cs[p] = cn[p]; sn[p] = snn[p]; }
       }
@@ -257,6 +230,21 @@ prep_fp32_kernel(PrepArgs a, int KT, int GC, int AC, int n_slabs, int n_chunks, 
   }
   if (tid < 3) cen[tid] = red[tid][0] / (double)a.n_ant;
   __syncthreads();
+  // range of the fixed-point phase reduction: |<p', r'>| <= |p'| rmax must stay below 2^19 turns; every block
+  // reaches the same verdict, and a collect that fails it contributes nothing (zero weights) and raises the flag
+  double far2 = 0.0;
+  for (int i = tid; i < a.n_ant; i += 256) {
+    const double dx = a.xyz[i] - cen[0], dy = a.xyz[i + a.ldxyz] - cen[1], dz = a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2];
+    far2 = fmax(far2, dx * dx + dy * dy + dz * dz);
+  }
+  red[0][tid] = far2;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) red[0][tid] = fmax(red[0][tid], red[0][tid + w]);
+    __syncthreads();
+  }
+  const bool in_range = sqrt(red[0][0]) / a.wavelength * a.rmax < kFp32PhaseLimit;
+  if (!in_range && blockIdx.x == 0 && tid == 0) atomicOr(a.status, BB_FLAG_RANGE);
 
   const int64_t gid = (int64_t)blockIdx.x * 256 + tid;
   const int64_t n_elem = (int64_t)n_ant_pad * n_eig_pad;
@@ -295,7 +283,7 @@ prep_fp32_kernel(PrepArgs a, int KT, int GC, int AC, int n_slabs, int n_chunks, 
   const int64_t n_w = (int64_t)a.n_levels * n_eig_pad;
   if (gid < n_w) {
     const int l = (int)(gid / n_eig_pad), k = (int)(gid - (int64_t)l * n_eig_pad);
-    a.weights[gid] = (k < a.n_eig) ? a.D[l + (size_t)k * a.ldd] : 0.f;
+    a.weights[gid] = (k < a.n_eig && in_range) ? a.D[l + (size_t)k * a.ldd] : 0.f;
   }
 }
 
@@ -330,10 +318,6 @@ Fp32Plan bb_fp32_plan(int n_ant, int n_eig, int n_levels) {
   else { p.KT = 32; p.PT = 2; p.GC = 4; }
   p.MINB = 2;
   p.AC = 32;
-  if (const char* e = getenv("BB_FP32_CFG")) {   // tuning experiments: "KT,PT,GC,MINB,AC"
-    int kt, pt, gc, mb, ac;
-    if (sscanf(e, "%d,%d,%d,%d,%d", &kt, &pt, &gc, &mb, &ac) == 5) { p.KT = kt; p.PT = pt; p.GC = gc; p.MINB = mb; p.AC = ac; }
-  }
   const int per_slab = p.GC * p.KT;
   p.n_slabs = (n_eig + per_slab - 1) / per_slab;
   p.n_chunks = (n_ant + p.AC - 1) / p.AC;
@@ -363,8 +347,6 @@ int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int /*sm_coun
   if (plan.KT == kt && plan.PT == pt && plan.GC == gc && plan.MINB == mb) return launch_variant<kt, pt, gc, mb>(plan, a, st, launches);
   BB_CASE(8, 4, 1, 2) BB_CASE(12, 4, 1, 2) BB_CASE(16, 4, 1, 2)
   BB_CASE(32, 2, 1, 2) BB_CASE(32, 2, 2, 2) BB_CASE(32, 2, 4, 2)
-  BB_CASE(16, 2, 4, 4) BB_CASE(16, 2, 4, 3) BB_CASE(32, 1, 2, 4) BB_CASE(32, 1, 2, 3) BB_CASE(16, 2, 2, 4) BB_CASE(16, 2, 1, 4)
-  BB_CASE(32, 2, 2, 3) BB_CASE(16, 4, 4, 2) BB_CASE(8, 4, 1, 4) BB_CASE(12, 2, 1, 4) BB_CASE(8, 2, 1, 4)
 #undef BB_CASE
   return BB_EUNSUPPORTED;
 }

@@ -36,8 +36,6 @@
 //              layout, written by prep_tc_kernel) global -> shared with cp.async.bulk on mbarriers.
 #include "internal.h"
 #include <cuda_fp16.h>
-#include <cstdio>
-#include <cstdlib>
 
 namespace {
 
@@ -232,14 +230,6 @@ __device__ __forceinline__ void split_f16(float c, float s, uint32_t& hi, uint32
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
-#ifdef BB_TC_TRACE
-__device__ long long g_trace[4][128][4];
-__device__ __forceinline__ long long clk64() { long long c; asm volatile("mov.u64 %0, %%clock64;" : "=l"(c)); return c; }
-#define TR(role, slot) do { if (blockIdx.x == 0 && n < 128) g_trace[role][n][slot] = clk64(); } while (0)
-#else
-#define TR(role, slot) do { } while (0)
-#endif
-
 // ---------------------------------------------------------------------------- synthesizer
 // Chunk in global/shared memory (N = 2 NE rows, kK columns of kElem bytes):
 //   [ B_hi : (kK*kElem/16) core columns x (N/8) row groups x (8 rows x 16 B) ][ B_lo : same ][ kAC antenna records ]
@@ -353,7 +343,6 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     for (int n = group;; n += 2) {
       const bool have = n < total;
       if (have) {
-        if (tid == 0) TR(0, 0);
         if constexpr (C::kLsOnTensor) {
           // ls_full(n) also implies that the MMAs which last read this A stage have completed (same issuer, in order)
           mbar_wait2(&b_full[sb], pb, &ls_full[2 * sa + tile], pa);
@@ -361,7 +350,6 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           mbar_wait2(&a_empty[sa], pa ^ 1, &b_full[sb], pb);
         }
         tc_fence_after();
-        if (tid == 0) TR(0, 2);
         const int4* rec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes);
         const uint32_t a_col = tmem_base + lane_field + kColA + (uint32_t)sa * kColsStage + (uint32_t)tile * 2 * C::kColsHalf;
         if constexpr (MODE == BB_TC_TF32) {
@@ -398,7 +386,6 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (tid == 0) TR(0, 3);
         if (lane == 0) mbar_arrive(&a_full[2 * sa + tile]);
       }
       sa += 2; if (sa >= kSA) { sa -= kSA; pa ^= 1; }
@@ -519,16 +506,13 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
-          if (t == 0) TR(1, 0);
           if (C::kLsOnTensor) {
             if (n + 2 < total) issue_mini();               // chunk n + 2 (its b_full wait covered chunk n two iterations ago)
-            if (t == 0) TR(1, 1);
             mbar_wait(&a_full[2 * sa + t], pa);
           } else {
             mbar_wait2(&b_full[sb], pb, &a_full[2 * sa + t], pa);
           }
           tc_fence_after();
-          if (t == 0) TR(1, 2);
           const uint64_t b_hi = desc0 + (uint64_t)((uint32_t)sb * chunk16);
           const uint64_t b_lo = b_hi + (uint64_t)half16;
           const uint32_t a_hi = tb + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
@@ -543,7 +527,6 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           if (!C::kLsOnTensor) tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
-          if (t == 0) TR(1, 3);
           if (++sa == kSA) { sa = 0; pa ^= 1; }
           if (++sb == kSB) { sb = 0; pb ^= 1; }
         }
@@ -555,9 +538,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       int sb = 0, e = 0, c = 0;
       uint32_t pb = 1;
       for (int n = 0; n < total; ++n) {
-        TR(2, 0);
         mbar_wait(&b_empty[sb], pb);
-        TR(2, 1);
         const unsigned char* src = packed + (size_t)e * packed_stride + slab_offset + (size_t)c * chunk_bytes;
         mbar_expect_tx(&b_full[sb], chunk_bytes);
         bulk_g2s(stage_base + (size_t)sb * chunk_bytes, src, chunk_bytes, &b_full[sb]);
@@ -608,6 +589,20 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   }
   if (tid < 3) cen[tid] = red[tid][0] / (double)a.n_ant;
   __syncthreads();
+  // range of the integer phase reduction: IH = rint(p' 2^8) must fit an int32, i.e. |p'_d| < 2^23 wavelengths; every
+  // block reaches the same verdict, and a collect that fails it contributes nothing (zero weights) and raises the flag
+  double far = 0.0;
+  for (int i = tid; i < a.n_ant; i += 256)
+    far = fmax(far, fmax(fabs(a.xyz[i] - cen[0]), fmax(fabs(a.xyz[i + a.ldxyz] - cen[1]), fabs(a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2]))));
+  __shared__ double redm[256];
+  redm[tid] = far;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) redm[tid] = fmax(redm[tid], redm[tid + w]);
+    __syncthreads();
+  }
+  const bool in_range = redm[0] / a.wavelength < kTcCoordLimit;
+  if (!in_range && blockIdx.x == 0 && tid == 0) atomicOr(a.status, BB_FLAG_RANGE);
   // FP16 mode: the column scale 2^ex puts the largest input component in [2^12, 2^13) (the phase fold can
   // grow a component by sqrt 2; FP16 overflows at 65504); the weights absorb 2^(-2 ex) exactly.
   int ex = 0;
@@ -697,7 +692,7 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   // weights [level][n_eig_pad]; FP16 mode: |E|^2 comes out scaled by 2^(2 ex)
   const float wscale = (float)ldexp(1.0, -2 * ex);
   for (int l = tid; l < a.n_levels; l += 256)
-    a.weights[(size_t)l * n_eig_pad + k] = (k < a.n_eig) ? a.D[l + (size_t)k * a.ldd] * wscale : 0.f;
+    a.weights[(size_t)l * n_eig_pad + k] = (k < a.n_eig && in_range) ? a.D[l + (size_t)k * a.ldd] * wscale : 0.f;
 }
 
 template <int MODE>
@@ -724,17 +719,6 @@ int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* laun
     BB_CUDA(cudaGetLastError());
     ++*launches;
   }
-#ifdef BB_TC_TRACE
-  if (getenv("BB_TC_TRACE")) {
-    cudaStreamSynchronize(st);
-    static long long h[4][128][4];
-    cudaMemcpyFromSymbol(h, g_trace, sizeof(h));
-    const long long t0 = h[0][0][0];
-    for (int n = 0; n < 128; ++n)
-      fprintf(stderr, "TR %3d P %6lld %6lld %6lld %6lld | M %6lld %6lld %6lld %6lld | L %6lld %6lld\n", n, h[0][n][0] - t0, h[0][n][1] - t0,
-              h[0][n][2] - t0, h[0][n][3] - t0, h[1][n][0] - t0, h[1][n][1] - t0, h[1][n][2] - t0, h[1][n][3] - t0, h[2][n][0] - t0, h[2][n][1] - t0);
-  }
-#endif
   return BB_OK;
 }
 

@@ -35,7 +35,9 @@ minmax_partial(const double* __restrict__ pix, int64_t n_pix, int64_t ld, double
   if (threadIdx.x < 6) part[blockIdx.x * 6 + threadIdx.x] = sm[threadIdx.x][0];
 }
 
+// rc[0..2] = centre of the bounding box, rc[3] = half its diagonal (>= max |r - r_c|)
 __global__ void minmax_final(const double* __restrict__ part, double* __restrict__ rc) {
+  __shared__ double half[3];
   if (threadIdx.x < 3) {
     double lo = DBL_MAX, hi = -DBL_MAX;
     for (int b = 0; b < kBlocks; ++b) {
@@ -43,7 +45,10 @@ __global__ void minmax_final(const double* __restrict__ part, double* __restrict
       hi = fmax(hi, part[b * 6 + 3 + threadIdx.x]);
     }
     rc[threadIdx.x] = 0.5 * (lo + hi);
+    half[threadIdx.x] = 0.5 * (hi - lo);
   }
+  __syncthreads();
+  if (threadIdx.x == 0) rc[3] = sqrt(half[0] * half[0] + half[1] * half[1] + half[2] * half[2]);
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -57,17 +62,20 @@ centre_pixels(const double* __restrict__ pix, int64_t n_pix, int64_t ld, const d
 }  // namespace
 
 int bb_pixels_prepare(const double* pix_dev, int64_t n_pix, int64_t ld_pix, double* rprime, int64_t pix_stride,
-                      double rc_out[3], cudaStream_t st) {
+                      double rc_out[3], double* rmax_out, cudaStream_t st) {
   double* scratch = nullptr;
-  BB_CUDA(cudaMalloc(&scratch, (kBlocks * 6 + 3) * sizeof(double)));
+  double host[4] = {0, 0, 0, 0};
+  BB_CUDA(cudaMalloc(&scratch, (kBlocks * 6 + 4) * sizeof(double)));
   minmax_partial<<<kBlocks, kThreads, 0, st>>>(pix_dev, n_pix, ld_pix, scratch);
   minmax_final<<<1, 32, 0, st>>>(scratch, scratch + kBlocks * 6);
   centre_pixels<<<(unsigned)((pix_stride + kThreads - 1) / kThreads), kThreads, 0, st>>>(
       pix_dev, n_pix, ld_pix, scratch + kBlocks * 6, rprime, pix_stride);
   cudaError_t e = cudaGetLastError();
-  if (e == cudaSuccess) e = cudaMemcpyAsync(rc_out, scratch + kBlocks * 6, 3 * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(host, scratch + kBlocks * 6, 4 * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(scratch);
+  rc_out[0] = host[0]; rc_out[1] = host[1]; rc_out[2] = host[2];
+  *rmax_out = host[3];
   if (e != cudaSuccess) { bb_note_cuda_error(e, "bb_pixels_prepare", __FILE__, __LINE__); return BB_ECUDA; }
   return BB_OK;
 }

@@ -17,3 +17,20 @@ def oracle():
     from oracle import bluebild_oracle
     bluebild_oracle.build()
     return bluebild_oracle
+
+
+def pytest_sessionfinish(session, exitstatus):
+    """Achieved parity errors (tests/helpers.record_parity) -> one JSON file, so that the numbers behind the
+    pass/fail verdicts are on file (profiles/ holds the copy of the last GPU run)."""
+    try:
+        import helpers
+    except Exception:
+        return
+    if not helpers.PARITY_RECORDS:
+        return
+    import json
+    path = os.environ.get("BB_PARITY_JSON", os.path.join(ROOT, "gpurun_out", "parity_errors.json"))
+    os.makedirs(os.path.dirname(path), exist_ok=True)
+    with open(path, "w") as f:
+        json.dump({"tolerance": {"rel_l2": helpers.REL_L2_TOL, "max_abs_over_peak": helpers.MAX_ABS_TOL},
+                   "records": helpers.PARITY_RECORDS}, f, indent=1)

@@ -413,6 +413,62 @@ def test_kmeans_levels_is_the_global_optimum(oracle, log_domain):
     assert lam[got == 0].min() > lam[got == 1].max() > lam[got == 2].max()     # level 0 = highest energy
 
 
+def _kmeans_spectra():
+    """Spectra for the contiguous-partition brute force: random, log-spread, exactly tied, nearly tied (1e-13
+    apart), and values that fall on what would be an edge of a coarser clustering."""
+    rng = np.random.default_rng(164)
+    out = []
+    for n in (5, 8, 11, 14):
+        out.append(rng.uniform(0.1, 10.0, n))
+        out.append(np.exp(rng.normal(0.0, 3.0, n)))
+        t = rng.uniform(1.0, 5.0, n)
+        t[1] = t[0]; t[-1] = t[-2]                                # exact ties
+        out.append(t)
+        nt = rng.uniform(1.0, 5.0, n)
+        nt[2] = nt[3] * (1.0 + 1e-13)                             # near tie
+        out.append(nt)
+        out.append(np.arange(1, n + 1, dtype=np.float64))         # equally spaced: many equal-cost splits
+        out.append(np.concatenate([[1.0, 2.0, 3.0], 3.0 + 2.0 ** -np.arange(n - 3)]))
+    out.append(np.array([1.0, 1.0, 1.0, 4.0, 4.0, 9.0, 9.0, 9.0, 9.0, 16.0, -2.0, 0.0]))
+    return out
+
+
+@pytest.mark.parametrize("log_domain", [False, True])
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
+def test_kmeans_levels_reaches_the_brute_force_minimum_over_contiguous_partitions(oracle, k, log_domain):
+    """PAPER.md:164, reading Q16. For n <= 14 every contiguous partition is enumerated with the cost written out
+    from its definition (helpers.kmeans_brute_contiguous); the oracle's intervals must induce a partition whose
+    cost equals that minimum and must be a valid level structure (helpers.kmeans_partition_check). An off-by-one
+    anywhere in a split search or its back-tracking yields a non-optimal or invalid partition and fails here."""
+    from helpers import kmeans_brute_contiguous, kmeans_partition_check
+    for lam in _kmeans_spectra():
+        pos = np.sort(lam[lam > 0])
+        if len(np.unique(pos)) < k:
+            continue
+        x = np.log(pos) if log_domain else pos
+        best = kmeans_brute_contiguous(x, k)
+        iv = oracle.kmeans_levels(lam, k, log_domain)
+        sse = kmeans_partition_check(lam, iv, k, log_domain)
+        assert sse <= best + 1e-12 * max(best, 1e-30) + 1e-13 * float(np.sum(x * x)), (k, log_domain, lam, sse, best)
+
+
+def test_kmeans_levels_all_assignments_four_clusters(oracle):
+    """All 4^8 assignments (contiguous or not) of 8 log-spread values to 4 clusters: the contiguity theorem the
+    oracle and the enumeration above rely on, checked where it can be."""
+    import itertools
+    from helpers import kmeans_partition_check
+    rng = np.random.default_rng(8)
+    lam = np.exp(rng.normal(0.0, 2.0, 8))
+    best = np.inf
+    for lab in itertools.product(range(4), repeat=8):
+        lab = np.array(lab)
+        if len(set(lab.tolist())) < 4:
+            continue
+        best = min(best, sum(np.sum((lam[lab == c] - lam[lab == c].mean()) ** 2) for c in range(4)))
+    sse = kmeans_partition_check(lam, oracle.kmeans_levels(lam, 4, False), 4, False)
+    assert abs(sse - best) <= 1e-12 * best
+
+
 def test_kmeans_levels_needs_enough_positive_values(oracle):
     with pytest.raises(ValueError):
         oracle.kmeans_levels([1.0, -2.0, 0.0], 2)
