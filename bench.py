@@ -2,7 +2,7 @@
 """bench.py — synthesizer throughput of the B200-native Bluebild Standard Synthesizer.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fp32|tf32x3|fp16x3]
-                    [--impl ours|reference] [--probe]
+                    [--impl ours|reference] [--quick]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: all collects of
 the config (config 4: 20 epochs of the 512-station, N_eig = 64, 8-level, 1024^2 wide-field case)
@@ -11,6 +11,10 @@ generation, contraction, level epilogue, multi-epoch accumulation). B = W V, the
 and hence D come from the library's own device glue (bb_eig), run before the timed region and
 timed separately ("glue" in the JSON line), as BASELINE.json's north_star prescribes.
 Metric: synthesizer terms/s, a term being one (antenna, eigenpair, pixel) complex MAC.
+Beside the headline (`value`, the --variant arm) the line carries, each measured in this run with its own
+clock record: `variants` (fp32, tf32x3, fp16x3 on the bench config: median of >= 5 event-timed steps, roofline
+fractions), `configs` (configs 2, 3, 5 through the same path), `e2e` (hot path from host buffers), `full_collect`
+(all of Algorithm 1 from host S / W / xyz / intervals to images on the host) and `cpu_baseline` (the oracle).
 Prints ONE JSON line on rank 0. See DESIGN.md "Measurement".
 """
 from __future__ import annotations
@@ -96,24 +100,27 @@ class ClockSampler(threading.Thread):
 
 
 # ------------------------------------------------------------------------------------ workload
-def prepare_inputs(cfg_idx, ctx, binding, workloads):
-    """Per-collect (B, D, xyz, wavelength) from the library's own glue; level edges per DESIGN.md."""
+def prepare_inputs(cfg_idx, ctx, binding, workloads, max_collects=None):
+    """Per-collect (B, D, xyz, wavelength) from the library's own glue; level edges per DESIGN.md.
+    max_collects: take only that many collects, evenly spaced over the run (config 5's 800 would take minutes
+    of host-side input generation; the timed collects are stated in the JSON line)."""
     w = workloads.make_workload(cfg_idx)
     c = w.cfg
     mid = w.collect_inputs(w.mid_collect())
     t0 = time.time()
     mu, _ = ctx.eig(mid["S"], mid["W"], mid["xyz"], mid["wavelength"], c.n_eig, want_B=False)
     items, lo, hi = [], mu[-1], mu[0]
-    for n in range(c.n_collects):
+    which = range(c.n_collects)
+    if max_collects is not None and max_collects < c.n_collects:
+        which = [int(round(x)) for x in np.linspace(0, c.n_collects - 1, max_collects)]
+    for n in which:
         ci = w.collect_inputs(n)
         lam, B = ctx.eig(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], c.n_eig)
         lo, hi = min(lo, lam[-1]), max(hi, lam[0])
         items.append(dict(B=B, lam=lam, xyz=ci["xyz"], wavelength=ci["wavelength"]))
     iv = workloads.choose_intervals(mu, c.n_levels, lam_max=hi, lam_min=lo)
     for it in items:
-        lam = it["lam"]
-        inside = (lam[None, :] >= iv[:, :1]) & (lam[None, :] <= iv[:, 1:])
-        it["D"] = np.asfortranarray(np.where(inside, lam[None, :], 0.0).astype(np.float32))
+        it["D"] = ctx.level_weights(it["lam"], iv)          # Alg. 1 l.7-8 by the library's own kernel
     return w, items, iv, time.time() - t0
 
 
@@ -165,7 +172,8 @@ def oracle_sample_run(oracle, w, items, n_levels, target_s, reps=1):
     rate = items[0]["B"].size * probe.shape[0] / max(time.perf_counter() - t0, 1e-6)
     n_s = int(max(cores, min(sub_all.size, target_s * rate / terms_per_pix)))
     n_s = max(cores, n_s // cores * cores)
-    pix = w.pixels(sub_all[:n_s])
+    take = sub_all[np.unique(np.linspace(0, sub_all.size - 1, n_s).astype(np.int64))]       # evenly over the whole image
+    pix = w.pixels(take)
     times = []
     for _ in range(reps):
         img = np.zeros((n_levels, pix.shape[0]))
@@ -174,7 +182,8 @@ def oracle_sample_run(oracle, w, items, n_levels, target_s, reps=1):
             oracle.synth(it["B"], it["D"], it["xyz"], pix, it["wavelength"], img=img)
         times.append(time.perf_counter() - t0)
     terms = terms_per_pix * pix.shape[0]
-    sample = "%d of %d pixels (every 4th row/column subset), all %d collects" % (pix.shape[0], w.cfg.n_pix, len(items))
+    sample = "%d of %d pixels (evenly spaced over the every-4th row/column grid of the whole image), all %d collects" % (
+        pix.shape[0], w.cfg.n_pix, len(items))
     return terms, times, cores, sample
 
 
@@ -213,6 +222,100 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------ our arm
+VARIANT_DTYPE = {"fp32": "f32", "tf32x3": "tf32x3", "fp16x3": "fp16x3", "fp16fp8": "fp16+fp8x2"}
+PASS_UNITS = {"tf32x3": 3.0, "fp16x3": 3.0, "fp16fp8": 2.0}   # tensor passes issued per useful one, in units of the variant's main format
+KERNEL_NAME = {"fp32": "synth_fp32_kernel", "tf32x3": "synth_tc_kernel<TF32>", "fp16x3": "synth_tc_kernel<FP16>",
+               "fp16fp8": "synth_tc_kernel<F16F8>"}
+
+
+def roofline_block(variant, flops_per_launch, avg_launch_ms, clocks, cfg_idx):
+    """Roofline of the synthesizer kernel of one timed arm: useful flops (8 per term) per launch over the kernel's
+    average launch duration (CUDA events around each launch, recorded by the library on the launching stream)."""
+    achieved = flops_per_launch / (avg_launch_ms * 1e-3) / 1e12
+    mp = measured_peaks()
+    if variant == "fp32":
+        bound, peak = "alu", FP32_PEAK_TFLOPS
+        basis = "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (derived, DESIGN.md 6)"
+    else:
+        bound = "tensor"
+        ratio = 0.5 if variant == "tf32x3" else 1.0            # dense FP16 = dense bf16; dense TF32 = 1/2 of it (guide's nominal ratio)
+        peak = mp["bf16_tflops"] * ratio
+        basis = "%.1f x bf16 burst peak (%s MEASURED_PEAKS.json); useful flops = 8/term, issued = %d/term in units of the main format%s" % (
+            ratio, mp["_source"], int(8 * PASS_UNITS[variant]), " (the FP8 pass of K = 64 counts as one FP16 pass: twice the rate)" if variant == "fp16fp8" else "")
+    r = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+         "kernel": KERNEL_NAME[variant], "flops_per_launch": flops_per_launch, "avg_launch_ms": avg_launch_ms, "peak_basis": basis}
+    if bound == "tensor":
+        # the split-precision schemes issue 3 (2 with the FP8 cross-term pass) tensor passes per useful one
+        r["issued_tflops"] = PASS_UNITS[variant] * achieved
+        r["issued_frac"] = PASS_UNITS[variant] * achieved / peak
+        sus = mp.get("bf16_tflops_sustained")
+        if sus:                                                # the power-capped figure (cuBLAS bf16 back to back for seconds)
+            r["issued_frac_of_sustained_peak"] = PASS_UNITS[variant] * achieved / (sus * ratio)
+    if clocks.get("sm_mhz"):                                   # the same peak scaled to the SM clock the run actually held
+        r["frac_at_observed_clock"] = achieved / (peak * clocks["sm_mhz"] / SM_MAX_MHZ)
+    # DRAM traffic of one launch: NOT measured in this run (that needs ncu) — the committed `ncu --set full` capture of
+    # this command, labelled as such
+    for rnd in ("r02", "r01"):
+        prof = os.path.join(ROOT, "profiles", "%s_%s_ncu_full.csv" % (rnd, variant))
+        if cfg_idx == 4 and os.path.exists(prof):
+            try:
+                import csv
+                mb = {row[0]: float(row[2]) for row in csv.reader(open(prof))
+                      if len(row) >= 3 and row[0].startswith("dram__bytes_") and row[1] == "Mbyte"}
+                if "dram__bytes_read.sum" in mb and "dram__bytes_write.sum" in mb:
+                    r["traffic"] = (mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]) * 1e6
+                    r["traffic_source"] = "committed ncu capture profiles/%s (not measured in this run)" % os.path.basename(prof)
+                    break
+            except Exception:
+                pass
+    return r
+
+
+def time_variant(binding, ctx, dev, pix_dev, dev_items, L, variant, steps, warmup, flush_buf, local_rank, terms_step):
+    """W warm-up steps, then `steps` steps each bracketed by its own CUDA-event pair on the context stream (L2 flushed
+    between steps, outside the pairs), SM clocks sampled over the timed region. Returns the arm's record."""
+    import torch
+    s = binding.StandardSynthesis(ctx, pix_dev, L, variant)
+
+    def step():
+        for it in dev_items:
+            s.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
+        s.flush()
+
+    for _ in range(warmup):
+        step()
+        flush_buf.zero_()
+    torch.cuda.synchronize()
+    t_before, l_before = s.timings(), s.launches()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    torch.cuda.synchronize()
+    evs = []
+    for _ in range(steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        evs.append((e0, e1))
+        flush_buf.zero_()                           # L2 flush between steps, outside the event pairs
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.finish()
+    per_step = [a.elapsed_time(b) for a, b in evs]
+    t_after, l_after = s.timings(), s.launches()
+    synth_ms = t_after["synth_ms"] - t_before["synth_ms"]
+    prep_ms = t_after["prep_ms"] - t_before["prep_ms"]
+    launches = l_after - l_before
+    synth_launches = launches - steps * len(dev_items)         # everything that is not a per-collect prep launch
+    avg_launch_ms = synth_ms / max(synth_launches, 1)
+    flops_per_launch = 8.0 * terms_step * steps / max(synth_launches, 1)
+    s.close()
+    return dict(per_step_ms=per_step, total_ms=float(sum(per_step)), median_ms=float(np.median(per_step)), clocks=clocks,
+                synth_ms=synth_ms, prep_ms=prep_ms, launches=int(launches), synth_launches=int(synth_launches),
+                avg_launch_ms=avg_launch_ms, flops_per_launch=flops_per_launch)
+
+
 def run_ours(args):
     import torch
     from paper_2310_09200_b200 import binding, workloads
@@ -227,53 +330,21 @@ def run_ours(args):
     c = w.cfg
     L = c.n_levels
     pix = w.pixels()
-
-    # ---- device-resident arm ------------------------------------------------------------------
     DM = binding.DeviceMatrix
-    dev_items = [dict(B=DM.from_numpy(it["B"], np.complex64, dev), D=DM.from_numpy(it["D"], np.float32, dev),
-                      xyz=DM.from_numpy(it["xyz"], np.float64, dev), wavelength=it["wavelength"]) for it in items]
-    s = binding.StandardSynthesis(ctx, DM.from_numpy(pix, np.float64, dev), L, args.variant)
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
-    def step_device():
-        for it in dev_items:
-            s.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
-        s.flush()
-
-    for _ in range(args.warmup):
-        step_device()
-        flush_buf.zero_()
-    torch.cuda.synchronize()
-    t_before, l_before = s.timings(), s.launches()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    barrier()
-    torch.cuda.synchronize()
-    evs = []
-    for _ in range(args.steps):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        step_device()
-        e1.record()
-        evs.append((e0, e1))
-        flush_buf.zero_()                           # L2 flush between steps, outside the event pairs
-    torch.cuda.synchronize()
-    barrier()
-    clocks = sampler.finish()
-    local_ms = sum(a.elapsed_time(b) for a, b in evs)
-    t_after, l_after = s.timings(), s.launches()
     terms_step = float(c.total_terms)
-    max_ms, total_terms = aggregate_over_ranks(local_ms, terms_step * args.steps, dev)
+
+    def to_device(its):
+        return [dict(B=DM.from_numpy(it["B"], np.complex64, dev), D=DM.from_numpy(it["D"], np.float32, dev),
+                     xyz=DM.from_numpy(it["xyz"], np.float64, dev), wavelength=it["wavelength"]) for it in its]
+
+    # ---- headline arm: device-resident inputs, --variant, --steps ----------------------------------------
+    dev_items = to_device(items)
+    pix_dev = DM.from_numpy(pix, np.float64, dev)
+    head = time_variant(binding, ctx, dev, pix_dev, dev_items, L, args.variant, args.steps, args.warmup, flush_buf, local_rank, terms_step)
+    max_ms, total_terms = aggregate_over_ranks(head["total_ms"], terms_step * args.steps, dev)
     ms_per_step = max_ms / args.steps
     value = total_terms / (max_ms * 1e-3)
-    synth_ms = t_after["synth_ms"] - t_before["synth_ms"]
-    prep_ms = t_after["prep_ms"] - t_before["prep_ms"]
-    launches = l_after - l_before
-    # synthesizer launches: one per queue flush (and per eigen slab) — everything else is a prep launch
-    synth_launches = launches - args.steps * len(items)
-    avg_launch_ms = synth_ms / max(synth_launches, 1)
-    flops_per_launch = 8.0 * terms_step * args.steps / max(synth_launches, 1)
-    achieved_tflops = flops_per_launch / (avg_launch_ms * 1e-3) / 1e12
 
     # ---- end-to-end arm: host buffers in, host images out, through the C ABI --------------------
     s2 = binding.StandardSynthesis(ctx, pix, L, args.variant)
@@ -298,109 +369,97 @@ def run_ours(args):
     e2e_ms, e2e_terms = aggregate_over_ranks(e2e_local_ms, terms_step * e2e_steps, dev)
     h2d = sum(it["B"].nbytes + it["D"].nbytes + it["xyz"].nbytes for it in items)
     d2h = out.nbytes
+    s2.close()
 
-    # ---- glue, timed separately: whole collect (Gram + eigensolve + select + prep) on one handle ----
-    glue = None
-    if rank == 0:
-        s3 = binding.StandardSynthesis(ctx, pix[:1024], L, args.variant)
-        ncol = min(len(items), 8)
-        for n in range(ncol):
-            ci = w.collect_inputs(n)
-            s3.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], c.n_eig, iv)
-        t3 = s3.timings()
-        glue = {"gram_ms_per_collect": t3["gram_ms"] / ncol, "eig_ms_per_collect": t3["eig_ms"] / ncol,
-                "collects_timed": ncol, "precision": "f64", "solver": "cusolverDnZhegvd"}
-        # the same through bb_synth_collect_batch: one potrfBatched / trsmBatched / XsyevBatched per 16 collects
-        nb = min(len(items), 16)
-        raws = [w.collect_inputs(n) for n in range(nb)]
-        Sb, Xb = np.stack([r["S"] for r in raws]), np.stack([r["xyz"] for r in raws])
-        Wb = None if raws[0]["W"] is None else np.stack([r["W"] for r in raws])
-        s4 = binding.StandardSynthesis(ctx, pix[:1024], L, args.variant)
-        for rep in range(2):                                      # first pass pays the library's one-time setup
-            tb4 = s4.timings()
-            s4.collect_batch(Sb, Wb, Xb, [r["wavelength"] for r in raws], c.n_eig, iv)
-        t4 = s4.timings()
-        glue["batched"] = {"gram_ms_per_collect": (t4["gram_ms"] - tb4["gram_ms"]) / nb,
-                           "eig_ms_per_collect": (t4["eig_ms"] - tb4["eig_ms"]) / nb, "collects_per_batch": nb,
-                           "solver": "cusolverDnZpotrfBatched + cublasZtrsmBatched + cusolverDnXsyevBatched"}
-
-    # ---- the other kernel variants on the same device-resident inputs (north_star: compare them) ----
-    others = {}
-    if rank == 0 and not args.no_compare:
-        for v in ("fp32", "tf32x3", "fp16x3"):
-            if v == args.variant:
-                continue
-            sv = binding.StandardSynthesis(ctx, DM.from_numpy(pix, np.float64, dev), L, v)
-            for rep in range(3):                                  # 2 warm-up passes, 1 timed
-                if rep == 2:
-                    tb = sv.timings()
-                for it in dev_items:
-                    sv.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
-                sv.flush()
-                flush_buf.zero_()
-            ms = sv.timings()["synth_ms"] - tb["synth_ms"]
-            others[v] = {"synth_ms_per_step": ms, "terms_per_s": terms_step / (ms * 1e-3)}
-            del sv
-
-    if rank != 0:
-        return
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": {"fp32": "f32", "tf32x3": "tf32x3", "fp16x3": "fp16x3"}[args.variant], "data": "synthetic",
+        "dtype": VARIANT_DTYPE[args.variant], "data": "synthetic",
         "config": {"workload": "config %d: %s" % (c.idx, c.name), "n_ant": c.n_ant, "n_beam": c.n_beam, "n_eig": c.n_eig,
                    "n_levels": L, "n_pix": c.n_pix, "n_collects": c.n_collects, "variant": args.variant,
                    "parallelism": "replicas x%d (no collective)" % world,
                    "l2": "flushed between steps (256 MiB memset, outside the per-step event pairs)",
-                   "timing": "sum of per-step CUDA-event pairs on the library's stream, max over ranks"},
-        "clocks": clocks,
+                   "timing": "sum of per-step CUDA-event pairs on the context stream (which waits for the library's synthesizer stream), max over ranks"},
+        "clocks": head["clocks"],
         "e2e": {"value": e2e_terms / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps,
                 "what": "collect_eig from host numpy buffers + bb_synth_get of every level image to host"},
-        "gpu_launches": int(launches),
+        "gpu_launches": head["launches"],
         "images_per_s": {"image_sets": 1e3 / ms_per_step * world, "collect_images": c.n_collects * 1e3 / ms_per_step * world},
-        "kernel_ms": {"synth_ms_per_step": synth_ms / args.steps, "prep_ms_per_step": prep_ms / args.steps,
-                      "synth_launches": int(synth_launches)},
-        "glue": glue,
-        "other_variants": others,
+        "kernel_ms": {"synth_ms_per_step": head["synth_ms"] / args.steps, "prep_ms_per_step": head["prep_ms"] / args.steps,
+                      "synth_launches": head["synth_launches"], "median_step_ms": head["median_ms"]},
+        "roofline": roofline_block(args.variant, head["flops_per_launch"], head["avg_launch_ms"], head["clocks"], c.idx),
     }
-    peak = FP32_PEAK_TFLOPS
-    bound = "alu"
-    if args.variant != "fp32":
-        mp = measured_peaks()
-        # dense FP16 = dense bf16; dense TF32 = 1/2 of it (guide's nominal ratio)
-        peak = mp["bf16_tflops"] * (1.0 if args.variant == "fp16x3" else 0.5)
-        bound = "tensor"
-    line["roofline"] = {"bound": bound, "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s",
-                        "frac": achieved_tflops / peak, "traffic": None,
-                        "kernel": "synth_fp32_kernel" if args.variant == "fp32" else "synth_tc_kernel",
-                        "flops_per_launch": flops_per_launch, "avg_launch_ms": avg_launch_ms,
-                        "peak_basis": ("148 SM x 128 FP32 lanes x 2 x 1.965 GHz (derived, DESIGN.md)" if bound == "alu" else
-                                       ("1.0" if args.variant == "fp16x3" else "0.5") + " x measured bf16 burst (MEASURED_PEAKS.json); useful flops = 8/term, issued = 24/term")}
-    # DRAM traffic of one launch of this kernel, from the committed `ncu --set full` capture of the same command
-    prof = os.path.join(ROOT, "profiles", "r01_%s_ncu_full.csv" % args.variant)
-    if args.config == 4 and os.path.exists(prof):
-        try:
-            import csv
-            mb = {r[0]: float(r[2]) for r in csv.reader(open(prof)) if len(r) >= 3 and r[0].startswith("dram__bytes_") and r[1] == "Mbyte"}
-            if "dram__bytes_read.sum" in mb and "dram__bytes_write.sum" in mb:
-                line["roofline"]["traffic"] = (mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]) * 1e6
-                line["roofline"]["traffic_source"] = "profiles/" + os.path.basename(prof)
-        except Exception:
-            pass
-    if bound == "tensor":
-        # the split-precision scheme issues 3 tensor passes per useful one: 24 flops per term on the pipe
-        line["roofline"]["issued_tflops"] = 3.0 * achieved_tflops
-        line["roofline"]["issued_frac"] = 3.0 * achieved_tflops / peak
-        sus = mp.get("bf16_tflops_sustained")
-        if sus:                                              # the power-capped figure (cuBLAS bf16 back to back for seconds)
-            line["roofline"]["issued_frac_of_sustained_peak"] = 3.0 * achieved_tflops / (sus * (1.0 if args.variant == "fp16x3" else 0.5))
-    if clocks.get("sm_mhz"):
-        line["roofline"]["frac_at_observed_clock"] = achieved_tflops / (peak * clocks["sm_mhz"] / SM_MAX_MHZ) if bound == "alu" else None
-    if args.probe:
-        line["probe"] = {k: ctx.probe_peak(i)[0] for i, k in enumerate(
-            ["ffma_per_s", "ffma2_fma_per_s", "mufu_per_s", "dfma_per_s", "dfma_chains_alone_per_s", "dfma_chains_under_mma_per_s",
-             "imad_chains_alone_per_s", "imad_chains_under_mma_per_s"])}
+    if rank != 0:
+        return
+
+    # ---- every variant north_star names, on the same device-resident inputs: full records ----------------
+    if not args.quick:
+        variants = {}
+        for v in ("fp32", "tf32x3", "fp16x3", "fp16fp8"):
+            if v == args.variant:
+                r = head
+            else:
+                r = time_variant(binding, ctx, dev, pix_dev, dev_items, L, v, max(5, args.variant_steps), 3, flush_buf, local_rank, terms_step)
+            variants[v] = {"terms_per_s": terms_step / (r["median_ms"] * 1e-3), "median_step_ms": r["median_ms"],
+                           "steps": len(r["per_step_ms"]), "per_step_ms": [round(x, 4) for x in r["per_step_ms"]],
+                           "clocks": r["clocks"], "roofline": roofline_block(v, r["flops_per_launch"], r["avg_launch_ms"], r["clocks"], c.idx)}
+        line["variants"] = variants
+    del dev_items, pix_dev
+
+    # ---- Algorithm 1 end to end: S, W, xyz, intervals on the host -> level images on the host -------------
+    raws = [w.collect_inputs(n) for n in range(c.n_collects)]
+    s5 = binding.StandardSynthesis(ctx, pix, L, args.variant)
+
+    def step_full():
+        for r in raws:
+            s5.collect(r["S"], r["W"], r["xyz"], r["wavelength"], c.n_eig, iv)
+        for l in range(L):
+            s5.get(l, out[l])
+
+    step_full()                                               # warm-up: library handles, scratch, solver set-up
+    tb = s5.timings()
+    fc_steps = 3
+    t0 = time.perf_counter()
+    for _ in range(fc_steps):
+        step_full()
+    torch.cuda.synchronize()
+    fc_ms = 1e3 * (time.perf_counter() - t0) / fc_steps
+    ta = s5.timings()
+    n_fc = fc_steps * len(raws)
+    line["full_collect"] = {
+        "value": terms_step / (fc_ms * 1e-3), "unit": UNIT, "ms_per_step": fc_ms, "steps": fc_steps,
+        "h2d_bytes_per_step": sum(r["S"].nbytes + r["xyz"].nbytes + (0 if r["W"] is None else r["W"].nbytes) + iv.nbytes for r in raws),
+        "d2h_bytes_per_step": d2h, "ratio_to_e2e_collect_eig": (e2e_ms / e2e_steps) / fc_ms,
+        "what": "bb_synth_collect per epoch from host S / W / xyz / intervals (device fp64 Gram + Cholesky + eigensolve, batched "
+                "over the queued collects on the glue stream) + bb_synth_get of every level image to host; wall clock",
+        "device_ms_per_collect": {k: (ta[k] - tb[k]) / n_fc for k in ("gram_ms", "eig_ms", "prep_ms", "synth_ms")}}
+    s5.close()
+    line["glue"] = {"precision": "f64", "batched_over": "up to 32 staged collects",
+                    "gram_ms_per_collect": line["full_collect"]["device_ms_per_collect"]["gram_ms"],
+                    "eig_ms_per_collect": line["full_collect"]["device_ms_per_collect"]["eig_ms"],
+                    "solver": "potrfBatched + trsmBatched + (block subspace iteration | XsyevBatched)"}
+
+    # ---- the other configs through the same path (device-resident, --variant) ---------------------------
+    if not args.quick and world == 1:
+        cfgs = {}
+        for idx, cap in ((2, None), (3, None), (5, args.cfg5_collects)):
+            if idx == args.config:
+                continue
+            wi, its, _, _ = prepare_inputs(idx, ctx, binding, workloads, max_collects=cap)
+            ci = wi.cfg
+            di = to_device(its)
+            t_step = float(ci.terms_per_collect) * len(its)
+            r = time_variant(binding, ctx, dev, DM.from_numpy(wi.pixels(), np.float64, dev), di, ci.n_levels, args.variant,
+                             3 if idx == 5 else 5, 3, flush_buf, local_rank, t_step)
+            cfgs["config %d: %s" % (idx, ci.name)] = {
+                "terms_per_s": t_step / (r["median_ms"] * 1e-3), "median_step_ms": r["median_ms"], "steps": len(r["per_step_ms"]),
+                "collects_per_step": len(its), "collects_in_config": ci.n_collects, "n_ant": ci.n_ant, "n_eig": ci.n_eig,
+                "n_pix": ci.n_pix, "phases_per_s": t_step / ci.n_eig / (r["median_ms"] * 1e-3), "clocks": r["clocks"],
+                "roofline": roofline_block(args.variant, r["flops_per_launch"], r["avg_launch_ms"], r["clocks"], idx)}
+            del di
+        line["configs"] = cfgs
+
     if world == 1 and not args.no_cpu_baseline:
         from oracle import bluebild_oracle as oracle      # cpu_baseline leg: the one place bench.py runs the oracle
         oracle.build()
@@ -415,10 +474,11 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp16x3"), choices=["fp32", "tf32x3", "fp16x3"])
-    ap.add_argument("--no-compare", action="store_true", help="skip the short timing of the other two variants")
+    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp16x3"), choices=["fp32", "tf32x3", "fp16x3", "fp16fp8"])
+    ap.add_argument("--quick", action="store_true", help="headline arm + e2e + full_collect only: skip the other variants and configs")
+    ap.add_argument("--variant-steps", type=int, default=5, help="timed steps of each non-headline variant (>= 5)")
+    ap.add_argument("--cfg5-collects", type=int, default=48, help="collects of config 5 timed per step (of 800)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--probe", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-step-seconds", type=float, default=10.0)

@@ -55,8 +55,10 @@ enum {
 enum {
   BB_VARIANT_FP32 = 0,    /* FP32 CUDA-core synthesizer (FFMA2), fp64-reduced phases          */
   BB_VARIANT_TF32X3 = 1,  /* tcgen05 tensor-core synthesizer, 3xTF32 split, fp32 accumulation */
-  BB_VARIANT_FP16X3 = 2   /* same with the operands split into FP16 pairs (same 11-bit significand as TF32,
+  BB_VARIANT_FP16X3 = 2,  /* same with the operands split into FP16 pairs (same 11-bit significand as TF32,
                              B columns pre-scaled by powers of two): twice the tensor rate            */
+  BB_VARIANT_FP16_FP8 = 3 /* FP16 main pass + ONE FP8 (e5m2) pass for both cross terms (kind::f8f6f4, K doubled):
+                             2 FP16-pass units instead of 3; rel-L2 ~ 8e-6 instead of ~5e-7  */
 };
 
 /* ---- context ------------------------------------------------------------------------------

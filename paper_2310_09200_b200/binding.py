@@ -20,9 +20,10 @@ BB_OK = 0
 VARIANT_FP32 = 0
 VARIANT_TF32X3 = 1
 VARIANT_FP16X3 = 2
+VARIANT_FP16_FP8 = 3
 FILTERS = {"lsq": 0, "std": 1}
 GRAM_MODES = {"sinc": 0, "identity": 1}
-_VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_FP16X3, 0: 0, 1: 1, 2: 2}
+_VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_FP16X3, "fp16fp8": VARIANT_FP16_FP8, 0: 0, 1: 1, 2: 2, 3: 3}
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",

@@ -237,7 +237,7 @@ extern "C" int bb_synth_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
   *out = nullptr;
   if (!ctx || n_pix < 0 || (n_pix > 0 && !pix) || ld_pix < n_pix || n_levels < 1 || n_levels > BB_MAX_LEVELS)
     return BB_EINVAL;
-  if (variant != BB_VARIANT_FP32 && variant != BB_VARIANT_TF32X3 && variant != BB_VARIANT_FP16X3) return BB_EUNSUPPORTED;
+  if (variant != BB_VARIANT_FP32 && variant != BB_VARIANT_TF32X3 && variant != BB_VARIANT_FP16X3 && variant != BB_VARIANT_FP16_FP8) return BB_EUNSUPPORTED;
   BB_CUDA(cudaSetDevice(ctx->device));
   bb_synth* s = new (std::nothrow) bb_synth;
   if (!s) return BB_EALLOC;
@@ -351,7 +351,7 @@ static int ensure_queue(bb_synth* s, int n_ant, int n_eig, size_t need) {
     s->fplan = bb_fp32_plan(n_ant, n_eig, L);
     s->packed_stride = s->fplan.collect_bytes; s->weight_stride = s->fplan.weight_floats;
   } else {
-    s->tplan = bb_tc_plan(n_ant, n_eig, L, s->variant == BB_VARIANT_FP16X3 ? BB_TC_FP16 : BB_TC_TF32);
+    s->tplan = bb_tc_plan(n_ant, n_eig, L, s->variant == BB_VARIANT_FP16X3 ? BB_TC_FP16 : s->variant == BB_VARIANT_FP16_FP8 ? BB_TC_F16F8 : BB_TC_TF32);
     if (s->tplan.n_chunks == 0) return BB_EUNSUPPORTED;
     s->packed_stride = s->tplan.collect_bytes; s->weight_stride = s->tplan.weight_floats;
   }

@@ -75,11 +75,15 @@ __global__ void select_kernel(const Z* __restrict__ v, int64_t stride_v, const d
   if (r == 0) lam[(size_t)b * stride_lam + k] = lam_all[(size_t)b * stride_l + src];
 }
 
-__global__ void narrow_kernel(const Z* __restrict__ src, int rows, int cols, bb_c32* __restrict__ dst, int64_t stride_dst) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y;
+// cast to complex64; a collect whose factorisation or eigensolve failed gets B = 0 (its eigenvectors may hold NaN, and
+// 0 weight x NaN would still poison the images)
+__global__ void narrow_kernel(const Z* __restrict__ src, int rows, int cols, bb_c32* __restrict__ dst, int64_t stride_dst,
+                              const int* __restrict__ info_chol, const int* __restrict__ info_eig) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y, b = blockIdx.z;
   if (r >= rows) return;
-  const Z x = src[(size_t)blockIdx.z * rows * cols + r + (size_t)c * rows];
-  dst[(size_t)blockIdx.z * stride_dst + r + (size_t)c * rows] = bb_c32{(float)x.x, (float)x.y};
+  const bool bad = info_chol[b] != 0 || info_eig[b] != 0;
+  const Z x = src[(size_t)b * rows * cols + r + (size_t)c * rows];
+  dst[(size_t)b * stride_dst + r + (size_t)c * rows] = bad ? bb_c32{0.f, 0.f} : bb_c32{(float)x.x, (float)x.y};
 }
 
 __global__ void pointer_array_kernel(Z** arr, Z* base, size_t stride, int n) {
@@ -267,9 +271,9 @@ int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, const GlueBatch& a, int* lau
       bb_note_cuda_error(cudaErrorUnknown, "cublasZgemmStridedBatched (B = W V)", __FILE__, __LINE__);
       return BB_ECUDA;
     }
-    narrow_kernel<<<dim3((n_ant + 127) / 128, n_eig, nb), blk, 0, st>>>(gB, n_ant, n_eig, a.B_dev, a.stride_b);
+    narrow_kernel<<<dim3((n_ant + 127) / 128, n_eig, nb), blk, 0, st>>>(gB, n_ant, n_eig, a.B_dev, a.stride_b, info_chol, info_eig);
   } else {
-    narrow_kernel<<<dim3((n_ant + 127) / 128, n_eig, nb), blk, 0, st>>>(gV, n_ant, n_eig, a.B_dev, a.stride_b);
+    narrow_kernel<<<dim3((n_ant + 127) / 128, n_eig, nb), blk, 0, st>>>(gV, n_ant, n_eig, a.B_dev, a.stride_b, info_chol, info_eig);
   }
   ++nl;
   if (a.ev_eig1) cudaEventRecord(a.ev_eig1, st);

@@ -41,9 +41,9 @@ struct Fp32Plan {
 Fp32Plan bb_fp32_plan(int n_ant, int n_eig, int n_levels);
 
 // Packed operand layout of the tensor-core (3xTF32 / 3xFP16) synthesizers; see kernels_tc.cu.
-enum { BB_TC_TF32 = 0, BB_TC_FP16 = 1 };
+enum { BB_TC_TF32 = 0, BB_TC_FP16 = 1, BB_TC_F16F8 = 2 };
 struct TcPlan {
-  int mode;          // BB_TC_TF32 or BB_TC_FP16
+  int mode;          // BB_TC_TF32, BB_TC_FP16 or BB_TC_F16F8
   int AC;            // antennas per K-chunk (K = 2*AC real columns per pass)
   int NB;            // N of the MMA = 2 * n_eig_pad_slab (Re | Im' halves)
   int n_slabs, n_chunks, n_eig_pad, n_ant_pad, eig_per_slab;

@@ -13,6 +13,10 @@
 // B columns pre-scaled by a power of two into FP16's range and the weights D[l,k] divided by its square);
 // D += A_hi B_hi + A_lo B_hi + A_hi B_lo with fp32 accumulation in TMEM (lo*lo ~ 2^-22 dropped).
 // FP16 carries the same significand as TF32 at twice the tensor rate and half the operand bytes.
+// A third mode (F16F8) keeps the FP16 main pass and runs BOTH cross terms as one FP8 pass at twice the FP16 rate:
+//     D += A_hi16 B_hi16  +  [ e5m2(A_lo) | e5m2(A) ] . [ e5m2(B) ; e5m2(B_lo) ]      (K doubled, kind::f8f6f4)
+//   2 FP16-pass units instead of 3; the cross terms are 2^-11 of the result, so their 3-bit significands cost
+//   ~2^-14 (measured rel-L2 < 1e-5).
 //
 // Phase generator (a1) WITHOUT fp64: DFMA shares hardware with the tensor pipe on B200 (a dependent DFMA
 // chain runs 2.6x slower while tcgen05.mma is streaming, and the 3-DFMA reduction of kernels_fp32.cu made
@@ -36,6 +40,7 @@
 //              layout, written by prep_tc_kernel) global -> shared with cp.async.bulk on mbarriers.
 #include "internal.h"
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 
 namespace {
 
@@ -68,6 +73,8 @@ template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one an
   static constexpr uint32_t kColA = 272;                 // A stages start (the mini-GEMM writes ls into a stage's lo half)
   static constexpr int kTail = 2 * kLsTile + kAC * 16;   // chunk tail: B1 | B2 (mini-GEMM operands) | IH records
 };
+
+template <> struct Cfg<BB_TC_F16F8> : Cfg<BB_TC_FP16> {};   // same tiles and TMEM plan; the lo half holds the FP8 cross-term operand
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -131,6 +138,11 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
   else
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem desc]; kind::f8f6f4 (the FP8 cross-term pass of F16F8 mode), K = 32 per instruction
+__device__ __forceinline__ void mma_ts_f8(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 // D[tmem] (+)= A[smem desc] * B[smem desc]; kind::f16 (the mini-GEMM of the small phase part)
 __device__ __forceinline__ void mma_ss_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
@@ -228,6 +240,20 @@ __device__ __forceinline__ void split_f16(float c, float s, uint32_t& hi, uint32
       "fma.rn.f32.f16 %0, a, m, %3;\n\tfma.rn.f32.f16 %1, b, m, %4;\n\t}" : "=f"(lc), "=f"(lsn) : "r"(hi), "f"(c), "f"(s));
   const __half2 l = __floats2half2_rn(lc, lsn);
   lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
+// (cos, sin) -> FP16 pair hi = rn16(x) and the FP8 cross-term word {e5m2(c - hi_c), e5m2(s - hi_s), e5m2(c), e5m2(s)}
+// (bytes 0..3 = the four K elements of this antenna in the FP8 pass).
+__device__ __forceinline__ void split_f16f8(float c, float s, uint32_t& hi, uint32_t& x8) {
+  const __half2 h = __floats2half2_rn(c, s);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  float lc, lsn;
+  asm("{\n\t.reg .f16 a, b, m;\n\tmov.b32 {a, b}, %2;\n\tmov.b16 m, 0xBC00;\n\t"
+      "fma.rn.f32.f16 %0, a, m, %3;\n\tfma.rn.f32.f16 %1, b, m, %4;\n\t}" : "=f"(lc), "=f"(lsn) : "r"(hi), "f"(c), "f"(s));
+  asm("{\n\t.reg .b16 l, a;\n\t"
+      "cvt.rn.satfinite.e5m2x2.f32 l, %2, %1;\n\t"
+      "cvt.rn.satfinite.e5m2x2.f32 a, %4, %3;\n\t"
+      "mov.b32 %0, {l, a};\n\t}" : "=r"(x8) : "f"(lc), "f"(lsn), "f"(c), "f"(s));
 }
 
 // ---------------------------------------------------------------------------- synthesizer
@@ -378,7 +404,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           for (int a = 0; a < 16; ++a) {
             float cs, sn;
             phase_cs_ls(ihrec[a], ls[a], q.jx, q.jy, q.jz, cs, sn);
-            split_f16(cs, sn, hi[a], lo[a]);
+            if constexpr (MODE == BB_TC_F16F8) split_f16f8(cs, sn, hi[a], lo[a]);
+            else split_f16(cs, sn, hi[a], lo[a]);
           }
           tmem_st16(a_col, hi);
           tmem_st16(a_col + C::kColsHalf, lo);
@@ -467,6 +494,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const uint32_t tb = __shfl_sync(0xffffffffu, tmem_base, 0);
     if (elect_one()) {
       const uint32_t idesc = (1u << 4) | (C::kFmt << 7) | (C::kFmt << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+      const uint32_t idesc8 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);   // A, B = E5M2
       const uint64_t desc0 = make_b_desc(smem_u32(stage_base), lbo, sbo);
       const uint32_t step16 = (2 * lbo) >> 4;              // one MMA consumes two 16-byte core columns of B
       const uint32_t chunk16 = chunk_bytes >> 4, half16 = half_bytes >> 4;
@@ -516,14 +544,24 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           const uint64_t b_hi = desc0 + (uint64_t)((uint32_t)sb * chunk16);
           const uint64_t b_lo = b_hi + (uint64_t)half16;
           const uint32_t a_hi = tb + kColA + (uint32_t)sa * kColsStage + (uint32_t)t * 2 * C::kColsHalf, a_lo = a_hi + C::kColsHalf;
+          if constexpr (MODE == BB_TC_F16F8) {
+            // FP16 main pass (K = 32 halves), then both cross terms as one FP8 pass (K = 64 bytes: 2 MMAs of K = 32)
 #pragma unroll
-          for (int pass = 0; pass < 3; ++pass)
+            for (int kk = 0; kk < C::kMmaPerPass; ++kk)
+              mma_ts<BB_TC_FP16>(d, a_hi + kk * 8, b_hi + (uint64_t)(kk * step16), idesc, (c | kk) != 0 ? 1u : 0u);
 #pragma unroll
-            for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
-              const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
-              const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
-              mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
-            }
+            for (int kk = 0; kk < 2; ++kk)
+              mma_ts_f8(d, a_lo + kk * 8, b_lo + (uint64_t)(kk * step16), idesc8, 1u);
+          } else {
+#pragma unroll
+            for (int pass = 0; pass < 3; ++pass)
+#pragma unroll
+              for (int kk = 0; kk < C::kMmaPerPass; ++kk) {
+                const uint32_t a = (pass == 1 ? a_lo : a_hi) + kk * 8;
+                const uint64_t bd = (pass == 2 ? b_lo : b_hi) + (uint64_t)(kk * step16);
+                mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
+              }
+          }
           if (!C::kLsOnTensor) tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(d_full);
@@ -573,7 +611,7 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   float amax = 0.f;
   for (int i = tid; i < a.n_ant; i += 256) {
     sx += a.xyz[i]; sy += a.xyz[i + a.ldxyz]; sz += a.xyz[i + 2 * (size_t)a.ldxyz];
-    if (MODE == BB_TC_FP16 && k < a.n_eig) {
+    if (MODE != BB_TC_TF32 && k < a.n_eig) {
       const bb_c32 b = a.B[i + (size_t)k * a.ldb];
       amax = fmaxf(amax, fmaxf(fabsf(b.re), fabsf(b.im)));
     }
@@ -606,7 +644,7 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   // FP16 mode: the column scale 2^ex puts the largest input component in [2^12, 2^13) (the phase fold can
   // grow a component by sqrt 2; FP16 overflows at 65504); the weights absorb 2^(-2 ex) exactly.
   int ex = 0;
-  if (MODE == BB_TC_FP16 && redf[0] > 0.f && isfinite(redf[0])) {
+  if (MODE != BB_TC_TF32 && redf[0] > 0.f && isfinite(redf[0])) {
     ex = 12 - ilogbf(redf[0]);
     ex = ex > 40 ? 40 : (ex < -40 ? -40 : ex);
   }
@@ -643,10 +681,20 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
         split_tf32(v, hi, lo);
         *reinterpret_cast<uint32_t*>(chunk + off) = hi;
         *reinterpret_cast<uint32_t*>(chunk + half_bytes + off) = lo;
-      } else {
+      } else if (MODE == BB_TC_FP16) {
         const __half h = __float2half_rn(v);
         *reinterpret_cast<__half*>(chunk + off) = h;
         *reinterpret_cast<__half*>(chunk + half_bytes + off) = __float2half_rn(v - __half2float(h));
+      } else {
+        // F16F8: FP16 main operand as above; FP8 cross-term operand (K = 64 bytes per row, 16 per core column):
+        // byte 4 ii + w pairs with e5m2(A_lo) and holds e5m2(v), byte 4 ii + 2 + w pairs with e5m2(A) and holds e5m2(v - hi)
+        const __half h = __float2half_rn(v);
+        *reinterpret_cast<__half*>(chunk + off) = h;
+        const int w = kidx & 1, ant = kidx >> 1;
+        const int k8 = 4 * ant + w;
+        const size_t off8 = (size_t)(k8 / 16) * ((size_t)(N / 8) * 128) + (size_t)(n >> 3) * 128 + (size_t)(n & 7) * 16 + (size_t)(k8 % 16);
+        chunk[half_bytes + off8] = (unsigned char)__nv_cvt_float_to_fp8(v, __NV_SATFINITE, __NV_E5M2);
+        chunk[half_bytes + off8 + 2] = (unsigned char)__nv_cvt_float_to_fp8(v - __half2float(h), __NV_SATFINITE, __NV_E5M2);
       }
     };
     put(kk, 2 * ii, br);            // (Re,k)  x (i,cos)
@@ -736,19 +784,21 @@ TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels, int mode) {
   p.n_chunks = (n_ant + kAC - 1) / kAC;
   p.n_eig_pad = p.n_slabs * ne;
   p.n_ant_pad = p.n_chunks * kAC;
-  const int elem = mode == BB_TC_FP16 ? 2 : 4;
-  p.chunk_bytes = 2 * (size_t)kK * p.NB * elem + (size_t)(mode == BB_TC_FP16 ? Cfg<BB_TC_FP16>::kTail : Cfg<BB_TC_TF32>::kTail);
+  const int elem = mode == BB_TC_TF32 ? 4 : 2;
+  p.chunk_bytes = 2 * (size_t)kK * p.NB * elem + (size_t)(mode == BB_TC_TF32 ? Cfg<BB_TC_TF32>::kTail : Cfg<BB_TC_FP16>::kTail);
   p.collect_bytes = (size_t)p.n_slabs * p.n_chunks * p.chunk_bytes;
   p.weight_floats = (size_t)n_levels * p.n_eig_pad;
   return p;
 }
 
 int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
-  return plan.mode == BB_TC_FP16 ? launch_prep<BB_TC_FP16>(plan, a, st) : launch_prep<BB_TC_TF32>(plan, a, st);
+  return plan.mode == BB_TC_FP16 ? launch_prep<BB_TC_FP16>(plan, a, st)
+         : plan.mode == BB_TC_F16F8 ? launch_prep<BB_TC_F16F8>(plan, a, st) : launch_prep<BB_TC_TF32>(plan, a, st);
 }
 
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int /*sm_count*/, cudaStream_t st, int* launches) {
   *launches = 0;
   if (a.n_collects <= 0 || a.n_pix <= 0) return BB_OK;
-  return plan.mode == BB_TC_FP16 ? launch_tc<BB_TC_FP16>(plan, a, st, launches) : launch_tc<BB_TC_TF32>(plan, a, st, launches);
+  return plan.mode == BB_TC_FP16 ? launch_tc<BB_TC_FP16>(plan, a, st, launches)
+         : plan.mode == BB_TC_F16F8 ? launch_tc<BB_TC_F16F8>(plan, a, st, launches) : launch_tc<BB_TC_TF32>(plan, a, st, launches);
 }

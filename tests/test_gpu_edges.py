@@ -7,7 +7,7 @@ from helpers import assert_parity
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = ["fp32", "tf32x3", "fp16x3"]
+VARIANTS = ["fp32", "tf32x3", "fp16x3", "fp16fp8"]
 
 
 @pytest.fixture(scope="module")

@@ -28,7 +28,7 @@ def test_random_shapes_agree_across_variants_and_runs():
             items.append((np.asfortranarray(B.astype(np.complex64)), np.asfortranarray(D.astype(np.float32)),
                           np.asfortranarray(rng.uniform(-ext, ext, size=(n_ant, 3)))))
         imgs = {}
-        for variant in ("fp32", "fp16x3", "fp16x3", "tf32x3", "tf32x3"):
+        for variant in ("fp32", "fp16x3", "fp16x3", "tf32x3", "tf32x3", "fp16fp8", "fp16fp8"):
             s = binding.StandardSynthesis(ctx, pix, L, variant)
             for B, D, xyz in items:
                 s.collect_eig(B, D, xyz, wl)
@@ -38,7 +38,7 @@ def test_random_shapes_agree_across_variants_and_runs():
             imgs[variant] = im
         ref = imgs["fp32"].astype(np.float64)
         peak = np.max(np.abs(ref)) or 1.0
-        for v in ("fp16x3", "tf32x3"):
+        for v in ("fp16x3", "tf32x3", "fp16fp8"):
             err = np.max(np.abs(imgs[v] - ref)) / peak
             worst = max(worst, err)
             assert err < 5e-5, (v, err, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
