@@ -136,7 +136,7 @@ class Context:
 
     def close(self):
         """Destroys the context; imaging handles created from it are closed first (bb_ctx_destroy refuses while any is alive)."""
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and _lib is not None:
             for ref in self._children:
                 child = ref()
                 if child is not None:

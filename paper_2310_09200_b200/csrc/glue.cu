@@ -64,8 +64,8 @@ __global__ void hermitian_fix_kernel(Z* __restrict__ a, int n) {  // in place: b
   m[c + (size_t)r * n] = make_cuDoubleComplex(re, -im);
 }
 
-// Column k of the selection is eigenpair order[k] of the solver's output (largest first, Alg. 1 l.4):
-// ascending full spectrum (n_vec = n_beam): order[k] = n_beam - 1 - k; descending leading block: order[k] = k.
+// Column k of the selection is the k-th largest eigenpair (Alg. 1 l.4) of the solver's output, n_vec pairs in
+// ascending order (the full spectrum, or the Ritz pairs of the leading block): source column n_vec - 1 - k.
 __global__ void select_kernel(const Z* __restrict__ v, int64_t stride_v, const double* __restrict__ lam_all, int64_t stride_l,
                               int n_beam, int n_vec, int ascending, int n_eig, Z* __restrict__ vsel, double* __restrict__ lam,
                               int64_t stride_lam) {
@@ -246,14 +246,14 @@ int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, const GlueBatch& a, int* lau
   if (!ok) { bb_note_cuda_error(cudaErrorUnknown, "batched Cholesky / trsm", __FILE__, __LINE__); return BB_ECUDA; }
   // leading n_eig pairs by block subspace iteration where that pays (large n_beam, n_eig << n_beam, decaying
   // spectrum); otherwise, or when it does not converge, the full batched eigensolve
-  int n_vec = n_beam, ascending = 1;
+  int n_vec = n_beam;
+  const int ascending = 1;                                 // both solvers return eigenvalues in ascending order
   const Z* vecs = gS;
   const double* lams = gLam;
   int64_t stride_v = (int64_t)bb2, stride_l = n_beam;
   int used_subspace = 0;
   if ((rc = bb_subspace_top_eigs(g, st, nb, n_beam, n_eig, gS, &vecs, &stride_v, &lams, &stride_l, &n_vec, &used_subspace, &nl)) != BB_OK) return rc;
-  if (used_subspace) ascending = 0;
-  else if ((rc = eig_full(g, st, nb, n_beam, gS, gLam, info_eig)) != BB_OK) return rc;
+  if (!used_subspace && (rc = eig_full(g, st, nb, n_beam, gS, gLam, info_eig)) != BB_OK) return rc;
   // ---- a0'': select, back-transform, beamform, cast
   select_kernel<<<dim3((n_beam + 127) / 128, n_eig, nb), blk, 0, st>>>(vecs, stride_v, lams, stride_l, n_beam, n_vec, ascending, n_eig, gV,
                                                                       a.lambda_dev, a.stride_lam); ++nl;
