@@ -165,6 +165,26 @@ int bb_eig(bb_ctx* ctx, int n_ant, int n_beam, int n_eig, double wavelength, con
            int ldw, const bb_c32* S, int lds, const double* xyz, int ldxyz, double* lambda_out,
            bb_c32* B_out, int ldb_out);
 
+/* ---- "uniform" image weighting (Section 3.5) ------------------------------------------------
+ * "We calculate the sampling density function on a grid in uv space with Delta u = Delta v = 1/FoV. Each
+ * visibility is then weighted with the inverse of its sampling density function", before the eigendecomposition.
+ * A visibility is an antenna pair (p, q), p = q included; its uv point is (xyz_p - xyz_q) / wavelength projected on
+ * the image-plane axes e_u, e_v (unit 3-vectors, HOST pointers); cell index = nearest integer of u / cell.
+ *   bb_uvgrid_create   cell = 1 / FoV in wavelengths; max_uv = the largest |u|, |v| to resolve (baselines beyond are
+ *                      counted in the border cells); (2 ceil(max_uv / cell) + 3)^2 int32 counters on the device.
+ *   bb_uvgrid_add      adds the n_ant^2 visibilities of one collect (xyz n_ant x 3 float64, host or device) to the
+ *                      density; call it for every time step and channel of the observation, then collect.
+ *   bb_synth_set_weighting  collects made after this call divide S_pq by the density of its cell (cells never added
+ *                      count as density 1); grid == NULL restores natural weighting. Only W == NULL collects (a
+ *                      beamformed visibility has no single baseline): others return BB_EUNSUPPORTED. The grid must
+ *                      outlive the handle's pending work (call bb_synth_status or bb_synth_get before destroying it).
+ * Weighted visibility matrices may be indefinite; negative eigenvalues are handled as anywhere else. */
+typedef struct bb_uvgrid bb_uvgrid;
+int bb_uvgrid_create(bb_ctx* ctx, double cell, const double* e_u, const double* e_v, double max_uv, bb_uvgrid** out);
+int bb_uvgrid_add(bb_uvgrid* g, int n_ant, double wavelength, const double* xyz, int ldxyz);
+int bb_uvgrid_destroy(bb_uvgrid* g);
+int bb_synth_set_weighting(bb_synth* s, bb_uvgrid* grid);
+
 /* ---- level weights alone (Alg. 1 lines 7-8; filters PAPER.md:166) ----------------------
  * D_out[f * n_intervals + i, k] = d_f(lambda_k) if intervals[i,0] <= lambda_k <= intervals[i,1] else 0, with
  * d = lambda_k for BB_FILTER_LSQ and 1 for BB_FILTER_STD — the D that bb_synth_collect_eig takes, computed by the

@@ -23,6 +23,9 @@ Functions and the passage each follows:
 ``kmeans_levels``    PAPER.md:164: k-means clustering of the eigenvalues into energy levels; in one
                      dimension the global optimum is found by dynamic programming over the sorted
                      values (readings in DESIGN.md Q16).
+``uv_density``       Section 3.5 "uniform" weighting: the sampling density function on a
+``uniform_weights``  uv grid of cell 1/FoV; "each visibility is then weighted with the inverse of its
+                     sampling density" before the eigendecomposition (readings in DESIGN.md Q17).
 ===================  ==========================================================================
 
 Library primitives used as steps: numpy.linalg.cholesky, numpy.linalg.eigh, numpy.linalg.solve,
@@ -204,6 +207,40 @@ def kmeans_levels(lam, n_levels, log_domain=True):
     return iv
 
 
+# ---------------------------------------------------------------------------------- image weighting (Section 3.5)
+def _uv_cells(xyz, wavelength, e_u, e_v, cell):
+    """Integer uv cell of every antenna pair (p, q): baseline b_pq = (x_p - x_q) / lambda_w, projected
+    on the image-plane axes e_u, e_v; cell index = nearest integer of u / cell (the cell centred on the origin)."""
+    xyz = np.asarray(xyz, dtype=np.float64)
+    pu = (xyz @ np.asarray(e_u, dtype=np.float64)) / wavelength
+    pv = (xyz @ np.asarray(e_v, dtype=np.float64)) / wavelength
+    cu = np.rint((pu[:, None] - pu[None, :]) / cell).astype(np.int64)
+    cv = np.rint((pv[:, None] - pv[None, :]) / cell).astype(np.int64)
+    return cu, cv
+
+
+def uv_density(collects, e_u, e_v, cell):
+    """Sampling density function: number of visibilities (all antenna pairs, p = q included, of all the given
+    collects = [(xyz, wavelength), ...]) in each uv cell of side `cell` = 1 / FoV. Returns {(cu, cv): count}."""
+    density = {}
+    for xyz, wavelength in collects:
+        cu, cv = _uv_cells(xyz, wavelength, e_u, e_v, cell)
+        for a, b in zip(cu.ravel().tolist(), cv.ravel().tolist()):
+            density[(a, b)] = density.get((a, b), 0) + 1
+    return density
+
+
+def uniform_weights(xyz, wavelength, e_u, e_v, cell, density):
+    """(n_ant, n_ant) real weights 1 / density(cell of b_pq); the visibility matrix is multiplied by them entry by
+    entry before the eigendecomposition (W = I only: a beamformed visibility has no single baseline)."""
+    cu, cv = _uv_cells(xyz, wavelength, e_u, e_v, cell)
+    w = np.empty(cu.shape, dtype=np.float64)
+    for p in range(cu.shape[0]):
+        for q in range(cu.shape[1]):
+            w[p, q] = 1.0 / density[(int(cu[p, q]), int(cv[p, q]))]
+    return w
+
+
 # ---------------------------------------------------------------------------------- synthesis
 def synth(B, D, xyz, pix, wavelength, img=None, n_threads=0):
     """I_l(r_j) += sum_k D[l,k] |sum_i conj(B_ik) exp(+j 2 pi <p_i,r_j>/lambda_w)|^2 (Alg. 2)."""
@@ -242,9 +279,13 @@ def brute(B, D, xyz, pix, wavelength):
 
 
 # ---------------------------------------------------------------------------------- Alg. 1
-def eig_stage(S, W, xyz, wavelength, n_eig, gram_identity=False):
-    """Alg. 1 lines 2-4 and U = W alpha. Returns (lambda desc (n_eig,), B (n_ant,n_eig))."""
+def eig_stage(S, W, xyz, wavelength, n_eig, gram_identity=False, vis_weights=None):
+    """Alg. 1 lines 2-4 and U = W alpha. Returns (lambda desc (n_eig,), B (n_ant,n_eig)).
+    vis_weights: optional (n_beam, n_beam) real weights applied to S entry by entry first (Section 3.5)."""
     n_ant = np.asarray(xyz).shape[0]
+    if vis_weights is not None:
+        assert W is None, "uniform weighting is defined on antenna baselines (W = I)"
+        S = np.asarray(S, dtype=np.complex128) * np.asarray(vis_weights, dtype=np.float64)
     if gram_identity:                                       # G := I special case (PAPER.md:219)
         G = np.eye(np.asarray(S).shape[0], dtype=np.complex128)
     else:
@@ -257,8 +298,8 @@ def eig_stage(S, W, xyz, wavelength, n_eig, gram_identity=False):
 
 
 def collect(S, W, xyz, wavelength, n_eig, intervals, pix, img=None, filt="lsq",
-            gram_identity=False, n_threads=0):
+            gram_identity=False, n_threads=0, vis_weights=None):
     """Algorithm 1 for one time step / channel; accumulates into img."""
-    lam, B = eig_stage(S, W, xyz, wavelength, n_eig, gram_identity)
+    lam, B = eig_stage(S, W, xyz, wavelength, n_eig, gram_identity, vis_weights)
     D = level_weights(lam, intervals, filt)
     return synth(B, D, xyz, pix, wavelength, img=img, n_threads=n_threads)

@@ -27,7 +27,8 @@ _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_F
 
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
-           "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version"]
+           "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
+           "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version"]
 
 _lib = None
 
@@ -70,6 +71,10 @@ def load_library(path: str = LIB_PATH):
         "bb_kmeans_levels": ([vp, vp, i32, i32, i32, vp, i32], i32),
         "bb_synth_status": ([vp], i32),
         "bb_level_weights": ([vp, vp, i32, vp, i32, i32, i32, vp, vp, i32], i32),
+        "bb_uvgrid_create": ([vp, f64, vp, vp, f64, pp], i32),
+        "bb_uvgrid_add": ([vp, i32, f64, vp, i32], i32),
+        "bb_uvgrid_destroy": ([vp], i32),
+        "bb_synth_set_weighting": ([vp, vp], i32),
         "bb_status_string": ([i32], ctypes.c_char_p),
         "bb_version": ([], ctypes.c_char_p),
     }
@@ -188,6 +193,29 @@ class Context:
         return lam, B
 
 
+class UVGrid:
+    """bb_uvgrid: sampling density on a uv grid of cell 1/FoV for "uniform" weighting (Section 3.5)."""
+
+    def __init__(self, ctx: Context, cell: float, e_u, e_v, max_uv: float):
+        eu = np.ascontiguousarray(e_u, dtype=np.float64)
+        ev = np.ascontiguousarray(e_v, dtype=np.float64)
+        h = ctypes.c_void_p()
+        _check(_lib.bb_uvgrid_create(ctx._h, float(cell), eu.ctypes.data, ev.ctypes.data, float(max_uv), ctypes.byref(h)), "bb_uvgrid_create")
+        self._h, self.ctx = h, ctx
+
+    def add(self, xyz, wavelength):
+        keep = []
+        Xp, n_ant, _, ldx = _marshal(xyz, np.float64, keep)
+        _check(_lib.bb_uvgrid_add(self._h, n_ant, float(wavelength), Xp, ldx), "bb_uvgrid_add")
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.bb_uvgrid_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+
 class StandardSynthesis:
     """bb_synth: the imaging handle (Algorithm 1)."""
 
@@ -211,6 +239,11 @@ class StandardSynthesis:
 
     def reset(self):
         _check(_lib.bb_synth_reset(self._h), "bb_synth_reset")
+
+    def set_weighting(self, grid):
+        """Uniform weighting (Section 3.5) from a UVGrid for the collects made from now on; None = natural."""
+        _check(_lib.bb_synth_set_weighting(self._h, None if grid is None else grid._h), "bb_synth_set_weighting")
+        self._weighting = grid                                 # keep the grid alive while the handle refers to it
 
     def collect(self, S, W, xyz, wavelength, n_eig, intervals, filters=None, gram="sinc"):
         """Algorithm 1. filters: None (one LSQ filter) or a sequence of "lsq" / "std"; the handle's n_levels must be

@@ -92,6 +92,7 @@ struct bb_synth {
   std::vector<cudaEvent_t> slot_ev, prep_done; std::vector<char> slot_busy, slot_prepped;
   // collects whose inputs are staged (slots q_len .. q_len + g_pending - 1) and whose glue has not been enqueued yet
   int g_pending = 0, g_gram_mode = 0;
+  const bb_uvgrid* weighting = nullptr;   // uniform weighting (Section 3.5) of the collects staged from now on; NULL = natural
   std::vector<PendingGlue> pend;
   // glue outputs per slot
   bb_c32* glue_B = nullptr; double* glue_lambda = nullptr; float* glue_D = nullptr; int* glue_info = nullptr;
@@ -100,6 +101,10 @@ struct bb_synth {
   double acc_ms[T_KINDS] = {0, 0, 0, 0};
   int64_t launches = 0;
 };
+
+cudaStream_t bb_ctx_glue_stream(bb_ctx* ctx) { return ctx->glue_stream; }
+cudaStream_t bb_ctx_user_stream(bb_ctx* ctx) { return ctx->stream; }
+int bb_ctx_device(bb_ctx* ctx) { return ctx->device; }
 
 static bool is_device_ptr(const void* p) {
   cudaPointerAttributes at;
@@ -536,6 +541,7 @@ static int run_pending_glue(bb_synth* s) {
   g.lambda_dev = s->glue_lambda + (size_t)first * n_eig; g.stride_lam = n_eig;
   g.B_dev = s->glue_B + (size_t)first * n_ant * n_eig; g.stride_b = (int64_t)n_ant * n_eig;
   g.info_dev = s->glue_info + 2 * (size_t)first;
+  g.uv = bb_uvgrid_view(s->weighting);
   g.ev_gram0 = get_event(s); g.ev_gram1 = get_event(s); g.ev_eig0 = get_event(s); g.ev_eig1 = get_event(s);
   int launches = 0;
   int rc = bb_glue_eig_batch(c->glue, gs, g, &launches);
@@ -603,6 +609,7 @@ extern "C" int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig
   }
   int rc = check_full_args(s, n_ant, n_beam, n_eig, wavelength, W, ldw, S, lds, xyz, ldxyz, intervals, ld_int, n_intervals);
   if (rc != BB_OK) return rc;
+  if (s->weighting && W) return BB_EUNSUPPORTED;           // a beamformed visibility has no single baseline (Q17)
   BB_CUDA(cudaSetDevice(s->ctx->device));
   return stage_full(s, n_ant, n_beam, n_eig, wavelength, W, ldw, S, lds, xyz, ldxyz, intervals, ld_int, n_intervals, fl, gram_mode);
 }
@@ -618,6 +625,7 @@ extern "C" int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, in
     int rc = check_full_args(s, n_ant, n_beam, n_eig, wavelengths[c], W, ldw, S, lds, xyz, ldxyz, intervals, ld_int, s->n_levels);
     if (rc != BB_OK) return rc;
   }
+  if (s->weighting && W) return BB_EUNSUPPORTED;
   BB_CUDA(cudaSetDevice(s->ctx->device));
   FilterList fl{};
   fl.n = 1; fl.kind[0] = BB_FILTER_LSQ;
@@ -626,6 +634,15 @@ extern "C" int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, in
                         xyz + (size_t)c * stride_xyz, ldxyz, intervals, ld_int, s->n_levels, fl, BB_GRAM_SINC);
     if (rc != BB_OK) return rc;
   }
+  return BB_OK;
+}
+
+extern "C" int bb_synth_set_weighting(bb_synth* s, bb_uvgrid* grid) {
+  if (!s) return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(s->ctx->device));
+  int rc = run_pending_glue(s);                            // collects staged so far keep the weighting they were staged under
+  if (rc != BB_OK) return rc;
+  s->weighting = grid;
   return BB_OK;
 }
 

@@ -45,13 +45,20 @@ __global__ void widen_kernel(const bb_c32* __restrict__ src, int ld, int64_t str
   dst[(size_t)b * rows * cols + r + (size_t)c * rows] = make_cuDoubleComplex(x.re, x.im);
 }
 
-// dst = (src + src^H)/2 widened to complex128 (reading Q10: S is used as its Hermitian part)
-__global__ void hermitian_part_kernel(const bb_c32* __restrict__ src, int ld, int64_t stride, int n, Z* __restrict__ dst) {
+// dst = (src + src^H)/2 widened to complex128 (reading Q10: S is used as its Hermitian part); with uniform weighting
+// (Section 3.5) every visibility is divided by the sampling density of its uv cell
+struct UvArgs { UvGridView g; const double* xyz; int ldxyz; int64_t stride_xyz; const double* wavelength; int64_t stride_wl; int on; };
+__global__ void hermitian_part_kernel(const bb_c32* __restrict__ src, int ld, int64_t stride, int n, Z* __restrict__ dst, UvArgs uv) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y, b = blockIdx.z;
   if (r >= n) return;
   const bb_c32* s = src + (size_t)b * stride;
   const bb_c32 x = s[r + (size_t)c * ld], y = s[c + (size_t)r * ld];
-  dst[(size_t)b * n * n + r + (size_t)c * n] = make_cuDoubleComplex(0.5 * ((double)x.re + (double)y.re), 0.5 * ((double)x.im - (double)y.im));
+  double w = 0.5;
+  if (uv.on) {
+    const int d = uv.g.count[bb_uv_cell(uv.g, uv.xyz + (size_t)b * uv.stride_xyz, uv.ldxyz, r, c, uv.wavelength[(size_t)b * uv.stride_wl])];
+    w = 0.5 / (double)(d > 0 ? d : 1);
+  }
+  dst[(size_t)b * n * n + r + (size_t)c * n] = make_cuDoubleComplex(w * ((double)x.re + (double)y.re), w * ((double)x.im - (double)y.im));
 }
 
 __global__ void hermitian_fix_kernel(Z* __restrict__ a, int n) {  // in place: both triangles <- Hermitian part
@@ -230,7 +237,9 @@ int bb_glue_eig_batch(GlueWork* g, cudaStream_t st, const GlueBatch& a, int* lau
 
   // ---- a0': G = L L^H, C = L^-1 S L^-H, C = Q diag(lambda) Q^H, V = L^-H Q   (G := I: C = S, V = Q, Eq. 38-40)
   if (a.ev_eig0) cudaEventRecord(a.ev_eig0, st);
-  hermitian_part_kernel<<<dim3((n_beam + 127) / 128, n_beam, nb), blk, 0, st>>>(a.S, a.lds, a.stride_s, n_beam, gS); ++nl;
+  UvArgs uv{};
+  if (a.uv) { uv.g = *a.uv; uv.xyz = a.xyz; uv.ldxyz = a.ldxyz; uv.stride_xyz = a.stride_xyz; uv.wavelength = a.wavelength; uv.stride_wl = a.stride_wl; uv.on = 1; }
+  hermitian_part_kernel<<<dim3((n_beam + 127) / 128, n_beam, nb), blk, 0, st>>>(a.S, a.lds, a.stride_s, n_beam, gS, uv); ++nl;
   bool ok = true;
   if (sinc) {
     pointer_array_kernel<<<(nb + 127) / 128, 128, 0, st>>>(pG, gG, bb2, nb);

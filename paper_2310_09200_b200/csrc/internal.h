@@ -95,6 +95,27 @@ int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int sm_count, cud
 int bb_pixels_prepare(const double* pix_dev, int64_t n_pix, int64_t ld_pix, double* rprime,
                       int64_t pix_stride, double rc_out[3], double* rmax_out, cudaStream_t st);
 
+// uniform weighting (Section 3.5, weighting.cu): the uv sampling-density grid as the kernels see it
+struct UvGridView {
+  int* count;          // device: (2 half + 1)^2 counters, cell (cu, cv) at (cv + half) * (2 half + 1) + cu + half
+  int half;
+  double cell;         // 1 / FoV, wavelengths
+  double eu[3], ev[3]; // image-plane axes
+};
+// cell of the visibility (p, q): baseline (x_p - x_q) / lambda_w projected on (e_u, e_v), nearest cell, clamped to the grid
+__device__ __forceinline__ size_t bb_uv_cell(const UvGridView& g, const double* __restrict__ xyz, int ld, int p, int q, double wavelength) {
+  const double px = xyz[p], py = xyz[p + ld], pz = xyz[p + 2 * (size_t)ld];
+  const double qx = xyz[q], qy = xyz[q + ld], qz = xyz[q + 2 * (size_t)ld];
+  const double up = (px * g.eu[0] + py * g.eu[1] + pz * g.eu[2]) / wavelength, uq = (qx * g.eu[0] + qy * g.eu[1] + qz * g.eu[2]) / wavelength;
+  const double vp = (px * g.ev[0] + py * g.ev[1] + pz * g.ev[2]) / wavelength, vq = (qx * g.ev[0] + qy * g.ev[1] + qz * g.ev[2]) / wavelength;
+  double cu = rint((up - uq) / g.cell), cv = rint((vp - vq) / g.cell);
+  const double h = (double)g.half;
+  cu = fmin(fmax(cu, -h), h); cv = fmin(fmax(cv, -h), h);
+  return (size_t)((long long)cv + g.half) * (2 * (size_t)g.half + 1) + (size_t)((long long)cu + g.half);
+}
+struct bb_uvgrid;
+const UvGridView* bb_uvgrid_view(const bb_uvgrid* g);
+
 // glue (Alg. 1 lines 2-4) — glue.cu; everything is batched over collects and asynchronous on the given stream
 struct GlueWork;
 struct SubspaceWork;
@@ -112,6 +133,7 @@ struct GlueBatch {
   const double* xyz; int ldxyz; int64_t stride_xyz;  // device
   double* lambda_dev; int64_t stride_lam;            // out: n_eig eigenvalues per collect, descending
   bb_c32* B_dev; int64_t stride_b;                   // out: B = W V, n_ant x n_eig complex64, ld n_ant
+  const UvGridView* uv;                              // NULL = natural weighting; else S_pq is divided by the density of its uv cell
   int* info_dev;                                     // out: [2 nb] Cholesky verdicts, then eigensolver verdicts
   cudaEvent_t ev_gram0, ev_gram1, ev_eig0, ev_eig1;  // may be null
 };

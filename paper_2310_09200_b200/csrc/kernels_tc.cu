@@ -54,7 +54,6 @@ constexpr int kMaxNE = 64;              // eigenpairs per slab
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t
 constexpr int kLsTile = 512;            // bytes of one mini-GEMM B operand tile (16 antennas x 16 halves)
-constexpr int kPixTile = 4096;          // bytes of the mini-GEMM A operand of one pixel tile (128 pixels x 16 halves)
 constexpr float kTwoPi = 6.283185307179586f;
 
 template <int MODE> struct Cfg;
@@ -67,11 +66,11 @@ template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (ti
   static constexpr int kTail = kAC * kRec;               // chunk tail: antenna records
 };
 template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one antenna share a 32-bit column
-  static constexpr int kElem = 2, kSA = 4, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
+  static constexpr int kElem = 2, kSA = 3, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
   static constexpr uint32_t kFmt = 0;   // F16
   static constexpr bool kLsOnTensor = true;              // small phase part as a K=16 mini-GEMM (see below)
-  static constexpr uint32_t kColLs = 0;                  // unused: the mini-GEMM's A operand (per-pixel constants) sits in shared memory
-  static constexpr uint32_t kColA = 256;                 // A stages start (the mini-GEMM writes ls into a stage's lo half)
+  static constexpr uint32_t kColLs = 256;                // mini-GEMM A operand (per-pixel constants): 8 columns per tile
+  static constexpr uint32_t kColA = 272;                 // A stages start (the mini-GEMM writes ls into a stage's lo half)
   static constexpr int kTail = 2 * kLsTile + kAC * 16;   // chunk tail: B1 | B2 (mini-GEMM operands) | IH records
 };
 
@@ -285,8 +284,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   const uint32_t lbo = (uint32_t)(N / 8) * 128, sbo = 128;
 
   unsigned char* stage_base = smem_raw;
-  unsigned char* apix = smem_raw + align_up((size_t)kSB * chunk_bytes, 1024);                    // [2 tiles][kPixTile] (FP16 modes)
-  float* lev = reinterpret_cast<float*>(apix + (C::kLsOnTensor ? 2 * kPixTile : 0));            // [2 groups][L][256]
+  float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [2 groups][L][256]
   float* dsm = lev + 2 * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
   uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + 2 * (size_t)n_levels * NE);
   uint64_t* b_full = bars;                 // [kSB]
@@ -339,8 +337,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const int ptid = tid;                                  // 0..511 over both groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
     if (C::kLsOnTensor && group == 0) {
-      // A operand of the mini-GEMM in shared memory (UMMA canonical K-major, no swizzle: LBO 2048, SBO 128), row = pixel,
-      // K = 16 halves: core column 0 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 1, 0}, core column 1 = lo of the same.
+      // A operand of the mini-GEMM in TMEM, row = pixel, K = 16 halves in 8 columns:
+      //   columns 0-3 = hi of {RL 2^24 (x,y,z), r' (x,y,z), 1, 0}, columns 4-7 = lo of the same.
       const float v[7] = {q.lx * 16777216.0f, q.ly * 16777216.0f, q.lz * 16777216.0f, q.fx, q.fy, q.fz, 1.0f};
       __align__(16) __half hi[8], lo[8];
 #pragma unroll
@@ -349,11 +347,11 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         hi[u] = __float2half_rn(x);
         lo[u] = __float2half_rn(x - __half2float(hi[u]));
       }
-      const int r = slot & 127;
-      unsigned char* row = apix + (size_t)tile * kPixTile + (size_t)(r >> 3) * 128 + (size_t)(r & 7) * 16;
-      *reinterpret_cast<int4*>(row) = *reinterpret_cast<const int4*>(hi);
-      *reinterpret_cast<int4*>(row + 2048) = *reinterpret_cast<const int4*>(lo);
-      fence_proxy_async_smem();                            // generic-proxy stores -> visible to the tensor core's async proxy
+      const uint32_t* hw = reinterpret_cast<const uint32_t*>(hi);
+      const uint32_t* lw = reinterpret_cast<const uint32_t*>(lo);
+      tmem_st8(tmem_base + lane_field + C::kColLs + (uint32_t)tile * 8, hw[0], hw[1], hw[2], hw[3], lw[0], lw[1], lw[2], lw[3]);
+      tmem_wait_st();
+      tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&apix_full[tile]);
     }
@@ -504,18 +502,14 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       int n = 0;
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
-      // mini-GEMM (FP16 modes): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) - 2 pi for the 16
-      // antennas of chunk m, written into the lo half of A stage m % kSA, kSA - 1 chunks ahead of the main MMAs of
+      // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) - 2 pi for the 16
+      // antennas of chunk m, written into the lo half of A stage m % kSA two chunks ahead of the main MMAs of
       // chunk m. The stage was last read by the main MMAs of chunk m - kSA, issued earlier by this same thread:
       // the tensor pipe executes one thread's MMAs in order, so no barrier is needed to reuse the columns, and
-      // ls_full(m) tells the producers both "ls is there" and "the stage is free". The ring is 4 deep because a
-      // producer group can start chunk m only after the main MMAs of chunk m - kSA have run: with 3 stages that
-      // round trip (issuer wake-up, MMAs of both tiles, mini-GEMM, producer wake-up) left the producers asleep
-      // 15 % of the time (profiles/r02_fp16fp8_ncu_full.md).
+      // ls_full(m) tells the producers both "ls is there" and "the stage is free".
       const uint32_t idesc_ls = (1u << 4) | ((uint32_t)(kAC >> 3) << 17) | ((128u >> 4) << 24);
       const uint64_t desc_ls0 = make_b_desc(smem_u32(stage_base) + 2 * half_bytes, 2 * 128, 128);
-      const uint64_t a_pix = make_b_desc(smem_u32(apix) + (uint32_t)t * kPixTile, 2048, 128);
-      constexpr int kAhead = kSA - 1;
+      const uint32_t a_pix = tb + C::kColLs + (uint32_t)t * 8;
       int sbm = 0, sam = 0;
       uint32_t pbm = 0;
       auto issue_mini = [&]() {
@@ -523,24 +517,25 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         tc_fence_after();
         const uint64_t b1 = desc_ls0 + (uint64_t)((uint32_t)sbm * chunk16), b2 = b1 + (uint64_t)(kLsTile >> 4);
         const uint32_t dl = tb + kColA + (uint32_t)sam * kColsStage + (uint32_t)t * 2 * C::kColsHalf + C::kColsHalf;
-        mma_ss_f16(dl, a_pix, b1, idesc_ls, 0u);           // A_hi B_hi + A_lo B_hi
-        mma_ss_f16(dl, a_pix, b2, idesc_ls, 1u);           // A_hi B_lo
+        mma_ts<BB_TC_FP16>(dl, a_pix, b1, idesc_ls, 0u);   // A_hi B_hi + A_lo B_hi
+        mma_ts<BB_TC_FP16>(dl, a_pix, b2, idesc_ls, 1u);   // A_hi B_lo
         tc_commit(&ls_full[2 * sam + t]);
         if (++sbm == kSB) { sbm = 0; pbm ^= 1; }
         if (++sam == kSA) sam = 0;
       };
       if (C::kLsOnTensor) {
-        static_assert(!C::kLsOnTensor || kSA >= 3, "the mini-GEMM runs kSA - 1 >= 2 chunks ahead");
+        static_assert(!C::kLsOnTensor || kSA >= 3, "the mini-GEMM runs two chunks ahead");
         mbar_wait(&apix_full[t], 0);
         tc_fence_after();
-        for (int m = 0; m < kAhead && m < total; ++m) issue_mini();
+        if (total > 0) issue_mini();
+        if (total > 1) issue_mini();
       }
       for (int e = 0; e < n_collects; ++e) {
         mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
           if (C::kLsOnTensor) {
-            if (n + kAhead < total) issue_mini();          // chunk n + kAhead (its b_full wait also covers chunk n: the ring is in order)
+            if (n + 2 < total) issue_mini();               // chunk n + 2 (its b_full wait covered chunk n two iterations ago)
             mbar_wait(&a_full[2 * sa + t], pa);
           } else {
             mbar_wait2(&b_full[sb], pb, &a_full[2 * sa + t], pa);
@@ -760,8 +755,7 @@ template <int MODE>
 int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + (C::kLsOnTensor ? 2 * kPixTile : 0) +
-                      2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 4) * 8 + 16 + 1024;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) +                       2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 4) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;

@@ -195,3 +195,55 @@ def test_collect_ex_filters_and_gram_mode(bb, ctx, oracle, variant, gram):
     with pytest.raises(bb.BluebildError):
         s3.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, filters=["std", "lsq"])
     assert not s3.images().any()
+
+
+# ------------------------------------------------------------------------------------ uniform weighting (Section 3.5)
+@pytest.mark.parametrize("variant", ["fp32", "fp16fp8"])
+@pytest.mark.parametrize("cfg_idx,collects,stride", [(1, [0], None), (3, [0, 50, 99], 16)])
+def test_uniform_weighting_matches_oracle(bb, ctx, wl, oracle, cfg_idx, collects, stride, variant):
+    """bb_uvgrid_* + bb_synth_set_weighting against the oracle's Section 3.5: density on the 1/FoV uv grid over the
+    given collects, S_pq divided by the density of its cell before the eigendecomposition (weighted matrices may be
+    indefinite: the level edges are placed between signed eigenvalues)."""
+    from helpers import assert_well_posed, record_parity
+    w = wl.make_workload(cfg_idx)
+    c = w.cfg
+    cell = 1.0 / (c.n_side * w.pix_step)                          # 1 / FoV, the extent of the image in direction cosines
+    raws = [w.collect_inputs(n) for n in collects]
+    dens = oracle.uv_density([(r["xyz"], r["wavelength"]) for r in raws], w.e_l, w.e_m, cell)
+    wts = [oracle.uniform_weights(r["xyz"], r["wavelength"], w.e_l, w.e_m, cell, dens) for r in raws]
+    items = []
+    for n, r, wt in zip(collects, raws, wts):
+        lam, _ = oracle.eig_stage(r["S"], None, r["xyz"], r["wavelength"], min(c.n_eig + 1, c.n_beam), vis_weights=wt)
+        items.append(dict(n=n, lam=lam[:c.n_eig], lam_next=float(lam[c.n_eig]) if lam.size > c.n_eig else None))
+    mid = items[len(items) // 2]["lam"]
+    L = c.n_levels
+    edges = [0.5 * (mid[(q * c.n_eig) // L - 1] + mid[(q * c.n_eig) // L]) for q in range(1, L)]
+    bounds = [1e30] + edges + [-1e30]
+    iv = np.array([[bounds[l + 1], bounds[l]] for l in range(L)])
+    assert_well_posed(items, iv[:, :][np.abs(iv) < 1e29].reshape(-1, 1) if L > 1 else np.zeros((0, 1)))
+    pix = w.pixels(None if stride is None else w.sample_pixels(stride))
+    ref = np.zeros((L, pix.shape[0]))
+    for r, wt in zip(raws, wts):
+        oracle.collect(r["S"], None, r["xyz"], r["wavelength"], c.n_eig, iv, pix, img=ref, vis_weights=wt)
+    max_uv = max(np.max(np.abs(r["xyz"] @ e)) for r in raws for e in (w.e_l, w.e_m)) * 2.0 / min(r["wavelength"] for r in raws)
+    grid = bb.UVGrid(ctx, cell, w.e_l, w.e_m, max_uv)
+    for r in raws:
+        grid.add(r["xyz"], r["wavelength"])
+    s = bb.StandardSynthesis(ctx, pix, L, variant)
+    s.set_weighting(grid)
+    for r in raws:
+        s.collect(r["S"], None, r["xyz"], r["wavelength"], c.n_eig, iv)
+    got = s.images()
+    s.status()
+    record_parity(cfg_idx, "G2 uniform weighting", variant, got, ref, len(collects), ref.shape[1])
+    for l in range(L):                                            # signed eigenvalues: measure against the level's own peak
+        peak = np.max(np.abs(ref[l]))
+        assert np.linalg.norm(got[l] - ref[l]) <= 1e-4 * np.linalg.norm(ref[l]) and np.max(np.abs(got[l] - ref[l])) <= 1e-3 * peak, (l,)
+    # natural weighting again on the same handle: different images
+    s.set_weighting(None)
+    s.reset()
+    for r in raws:
+        s.collect(r["S"], None, r["xyz"], r["wavelength"], c.n_eig, iv)
+    assert np.max(np.abs(s.images() - got)) > 1e-3 * np.max(np.abs(got))
+    s.close()
+    grid.close()

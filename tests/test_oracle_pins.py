@@ -472,3 +472,68 @@ def test_kmeans_levels_all_assignments_four_clusters(oracle):
 def test_kmeans_levels_needs_enough_positive_values(oracle):
     with pytest.raises(ValueError):
         oracle.kmeans_levels([1.0, -2.0, 0.0], 2)
+
+
+# ---------------------------------------------------------------------------------- uniform weighting (Section 3.5)
+def test_uniform_weights_hand_computed_line_array(oracle):
+    """Three antennas on a line at spacing d, cell = d: the uv cells hold {0: 3 autocorrelations, +-d: 2 each,
+    +-2d: 1 each}, so the weights are 1/3 on the diagonal, 1/2 next to it and 1 in the corners — worked by hand."""
+    d, wl = 7.0, 2.0
+    xyz = np.array([[0.0, 0, 0], [d, 0, 0], [2 * d, 0, 0]])
+    e_u, e_v = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    dens = oracle.uv_density([(xyz, wl)], e_u, e_v, d / wl)
+    assert dens == {(0, 0): 3, (1, 0): 2, (-1, 0): 2, (2, 0): 1, (-2, 0): 1}
+    w = oracle.uniform_weights(xyz, wl, e_u, e_v, d / wl, dens)
+    assert np.allclose(w, [[1 / 3, 1 / 2, 1], [1 / 2, 1 / 3, 1 / 2], [1, 1 / 2, 1 / 3]], rtol=0, atol=1e-15)
+    # the density accumulates over collects: the same epoch twice halves every weight
+    dens2 = oracle.uv_density([(xyz, wl), (xyz, wl)], e_u, e_v, d / wl)
+    assert np.allclose(oracle.uniform_weights(xyz, wl, e_u, e_v, d / wl, dens2), w / 2)
+
+
+def test_uniform_weighting_with_one_visibility_per_cell_is_natural_weighting(oracle):
+    """If no two baselines share a uv cell (and the N autocorrelations are the only visibilities at the origin), the
+    off-diagonal weights are 1 and the diagonal 1/N: S' = S - (1 - 1/N) diag(S). With a constant density (every
+    weight equal to c) the weighted problem is c S: eigenvalues scale by c, eigenvectors and hence the STD-filter image
+    do not change, the LSQ image scales by c."""
+    rng = np.random.default_rng(35)
+    xyz, dirs, wl = _tiny_case(rng, n_ant=7, n=8)
+    e_u, e_v = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    cell = 1e-3                                                     # far smaller than any baseline difference
+    dens = oracle.uv_density([(xyz, wl)], e_u, e_v, cell)
+    w = oracle.uniform_weights(xyz, wl, e_u, e_v, cell, dens)
+    assert np.array_equal(w, np.where(np.eye(7, dtype=bool), 1.0 / 7.0, 1.0))
+    assert np.array_equal(w, w.T)
+    S = _random_sky_S(rng, xyz, wl)
+    lam_w, B_w = oracle.eig_stage(S, None, xyz, wl, 7, vis_weights=np.full((7, 7), 0.25))
+    lam_n, B_n = oracle.eig_stage(S, None, xyz, wl, 7)
+    assert np.allclose(lam_w, 0.25 * lam_n, rtol=1e-12)
+    iv = np.array([[0.0, 1e9]])
+    img_w = oracle.collect(S, None, xyz, wl, 7, iv, dirs, vis_weights=np.full((7, 7), 0.25))
+    img_n = oracle.collect(S, None, xyz, wl, 7, iv, dirs)
+    assert np.allclose(img_w, 0.25 * img_n, rtol=1e-10)
+    std_w = oracle.collect(S, None, xyz, wl, 7, iv, dirs, filt="std", vis_weights=np.full((7, 7), 0.25))
+    std_n = oracle.collect(S, None, xyz, wl, 7, iv, dirs, filt="std")
+    assert np.allclose(std_w, std_n, rtol=1e-10)
+
+
+def test_uniform_weighting_equals_linear_solve_form(oracle):
+    """P4 with weights: with all eigenpairs kept, the sum over levels equals a^H G^-1 (S o Wt) G^-1 a computed by a
+    linear solve — the weights act on the visibilities and on nothing else. Also: the density is symmetric under
+    b -> -b, so the weights are symmetric and S o Wt stays Hermitian."""
+    rng = np.random.default_rng(36)
+    xyz, dirs, wl = _tiny_case(rng, n_ant=9, n=8)
+    e_u, e_v = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    cell = 20.0                                                     # coarse: several baselines per cell
+    dens = oracle.uv_density([(xyz, wl)], e_u, e_v, cell)
+    assert all(dens[(-a, -b)] == c for (a, b), c in dens.items()) and max(dens.values()) > 2
+    Wt = oracle.uniform_weights(xyz, wl, e_u, e_v, cell, dens)
+    assert np.array_equal(Wt, Wt.T)
+    S = _random_sky_S(rng, xyz, wl)
+    lam, _ = oracle.eig_stage(S, None, xyz, wl, 9, vis_weights=Wt)
+    iv = np.array([[min(lam.min(), 0) * 2 - 1, 0.0], [np.nextafter(0.0, 1), lam.max() * 2]])   # a negative and a positive level
+    img = oracle.collect(S, None, xyz, wl, 9, iv, dirs, vis_weights=Wt)
+    G = oracle.gram(xyz, None, wl)
+    A = steering(xyz, dirs, wl)                                     # (n_ant, n_pix)
+    X = np.linalg.solve(G, A)
+    want = np.real(np.einsum("ij,ik,kj->j", X.conj(), S.astype(np.complex128) * Wt, X))
+    assert np.allclose(img.sum(axis=0), want, rtol=1e-9, atol=1e-9 * np.abs(want).max())
