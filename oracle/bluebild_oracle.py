@@ -23,6 +23,9 @@ Functions and the passage each follows:
 ``kmeans_levels``    PAPER.md:164: k-means clustering of the eigenvalues into energy levels; in one
                      dimension the global optimum is found by dynamic programming over the sorted
                      values (readings in DESIGN.md Q16).
+``gram_corrected_visibilities``  Eq. 17 / Eq. 21: V'_l = A Lambda_l A^H per level.
+``nufft_direct``     Eq. 18-19: the NUFFT-synthesis image as the literal double sum over
+                     baselines and pixels (what a type-3 NUFFT approximates); tiny inputs only.
 ``uv_density``       Section 3.5 "uniform" weighting: the sampling density function on a
 ``uniform_weights``  uv grid of cell 1/FoV; "each visibility is then weighted with the inverse of its
                      sampling density" before the eigendecomposition (readings in DESIGN.md Q17).
@@ -276,6 +279,31 @@ def brute(B, D, xyz, pix, wavelength):
                          _dptr(D), max(n_levels, 1), _dptr(xyz), max(n_ant, 1), _dptr(pix),
                          max(n_pix, 1), float(wavelength), _dptr(img))
     return img
+
+
+# ---------------------------------------------------------------------------------- NUFFT synthesis, direct form
+def gram_corrected_visibilities(B, D):
+    """Eq. 17 with the level selection of Eq. 21: V'_l = B diag(D[l, :]) B^H, one (n_ant, n_ant) matrix per level
+    ("constructed by setting eigenvalues which fall outside the interval to zero"; B = W alpha, Eq. 22-24)."""
+    B = np.asarray(B, dtype=np.complex128)
+    D = np.atleast_2d(np.asarray(D, dtype=np.float64))
+    return np.stack([(B * D[l][None, :]) @ B.conj().T for l in range(D.shape[0])])
+
+
+def nufft_direct(B, D, xyz, pix, wavelength):
+    """Eq. 18-19: I_l(r_j) = sum_p sum_q V'_l,pq exp(-2 pi i <b_pq, r_j>), b_pq = (x_p - x_q) / lambda_w — the sum a
+    type-3 NUFFT evaluates approximately, written out over all N_A^2 baselines. Returns (images (L, n_pix) real part,
+    largest |imaginary part|): the sum is real because V' is Hermitian and b_qp = -b_pq."""
+    V = gram_corrected_visibilities(B, D)
+    xyz = np.asarray(xyz, dtype=np.float64)
+    pix = np.asarray(pix, dtype=np.float64)
+    n_ant = xyz.shape[0]
+    img = np.zeros((V.shape[0], pix.shape[0]), dtype=np.complex128)
+    for p in range(n_ant):
+        for q in range(n_ant):
+            b = (xyz[p] - xyz[q]) / wavelength
+            img += V[:, p, q][:, None] * np.exp(-2j * np.pi * (pix @ b))[None, :]
+    return img.real, float(np.max(np.abs(img.imag)))
 
 
 # ---------------------------------------------------------------------------------- Alg. 1

@@ -537,3 +537,37 @@ def test_uniform_weighting_equals_linear_solve_form(oracle):
     X = np.linalg.solve(G, A)
     want = np.real(np.einsum("ij,ik,kj->j", X.conj(), S.astype(np.complex128) * Wt, X))
     assert np.allclose(img.sum(axis=0), want, rtol=1e-9, atol=1e-9 * np.abs(want).max())
+
+
+# ---------------------------------------------------------------------------------- NUFFT synthesis, direct form (oracle slice)
+def test_nufft_direct_equals_standard_synthesis(oracle):
+    """Eq. 16: Psi V' Psi^* = sum_a lambda_a |eps_a|^2 — the baseline-domain double sum (Eq. 18-19, 21) and Standard
+    Synthesis (Eq. 15, 20) evaluate the same images; also with a beamforming matrix and a standardized filter."""
+    rng = np.random.default_rng(44)
+    xyz, pix, wl = _tiny_case(rng, n_ant=6, n=6)
+    Wb = (rng.normal(size=(6, 4)) + 1j * rng.normal(size=(6, 4)))
+    for W in (None, Wb):
+        S = _random_sky_S(rng, xyz, wl, W=W)
+        lam, B = oracle.eig_stage(S, W, xyz, wl, S.shape[0])
+        iv = np.array([[lam[1] * 0.999, 1e9], [0.0, lam[1] * 0.999]])
+        for filt in ("lsq", "std"):
+            D = oracle.level_weights(lam, iv, filt)
+            want = oracle.synth(B, D, xyz, pix, wl)
+            got, imag = oracle.nufft_direct(B, D, xyz, pix, wl)
+            assert np.allclose(got, want, rtol=1e-11, atol=1e-11 * np.abs(want).max())
+            assert imag <= 1e-11 * np.abs(want).max()
+
+
+def test_nufft_direct_two_antennas_by_hand(oracle):
+    """V' = [[a, c], [conj(c), b]], baseline d along x: I(l) = a + b + 2 Re(c exp(-2 pi i d l / lambda)) — typed by hand."""
+    d, wl = 9.0, 3.0
+    xyz = np.array([[d, 0.0, 0.0], [0.0, 0.0, 0.0]])
+    l = np.linspace(-0.3, 0.3, 25)
+    pix = np.column_stack([l, np.zeros_like(l), np.sqrt(1 - l * l)])
+    B = np.array([[0.7 + 0.2j, 0.1 - 0.4j], [-0.3 + 0.5j, 0.6 + 0.1j]])
+    D = np.array([[2.0, 0.5]])
+    V = oracle.gram_corrected_visibilities(B, D)[0]
+    assert np.allclose(V, V.conj().T)
+    want = V[0, 0].real + V[1, 1].real + 2 * np.real(V[0, 1] * np.exp(-2j * np.pi * d * l / wl))
+    got, imag = oracle.nufft_direct(B, D, xyz, pix, wl)
+    assert np.allclose(got[0], want, rtol=1e-13, atol=1e-13) and imag < 1e-13
