@@ -474,7 +474,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp16x3"), choices=["fp32", "tf32x3", "fp16x3", "fp16fp8"])
+    ap.add_argument("--variant", default=os.environ.get("BB_VARIANT", "fp16fp8"), choices=["fp32", "tf32x3", "fp16x3", "fp16fp8"])
     ap.add_argument("--quick", action="store_true", help="headline arm + e2e + full_collect only: skip the other variants and configs")
     ap.add_argument("--variant-steps", type=int, default=5, help="timed steps of each non-headline variant (>= 5)")
     ap.add_argument("--cfg5-collects", type=int, default=48, help="collects of config 5 timed per step (of 800)")

@@ -50,22 +50,25 @@ _lib = None
 C_LIGHT = 299792458.0  # m/s; wavelength = c / f (reading Q3: PAPER.md:117 prints "f/c")
 
 
-def build(force: bool = False) -> str:
-    """Compile oracle/*.cpp into oracle/liboracle.so (g++ -O2, no fast-math)."""
+def build(force: bool = False, sanitize: bool = False) -> str:
+    """Compile oracle/*.cpp into oracle/liboracle.so (g++ -O2, no fast-math). sanitize=True builds
+    oracle/liboracle_san.so with AddressSanitizer + UndefinedBehaviorSanitizer instead (tests/test_sanitizers.py)."""
     srcs = [os.path.join(_HERE, s) for s in _SOURCES]
-    if (not force and os.path.exists(_LIB_PATH)
-            and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(s) for s in srcs)):
-        return _LIB_PATH
-    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", _LIB_PATH] + srcs
+    out = os.path.join(_HERE, "liboracle_san.so") if sanitize else _LIB_PATH
+    if (not force and os.path.exists(out)
+            and all(os.path.getmtime(out) >= os.path.getmtime(s) for s in srcs)):
+        return out
+    flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if sanitize else ["-O2"]
+    cmd = ["g++"] + flags + ["-std=c++17", "-fPIC", "-shared", "-pthread", "-o", out] + srcs
     subprocess.run(cmd, check=True)
-    return _LIB_PATH
+    return out
 
 
 def _load():
     global _lib
     if _lib is None:
-        build()
-        lib = ctypes.CDLL(_LIB_PATH)
+        path = build(sanitize=True) if os.environ.get("BB_ORACLE_SANITIZE") else build()
+        lib = ctypes.CDLL(path)
         dp = ctypes.POINTER(ctypes.c_double)
         lib.oracle_synth.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int64,
                                      dp, ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int,
