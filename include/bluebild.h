@@ -89,8 +89,8 @@ int bb_synth_reset(bb_synth* s); /* drop pending collects and zero the level ima
  *   xyz n_ant x 3 float64 metres, ld ldxyz (P_icrs of Table 1)
  *   intervals n_levels x 2 float64, ld ld_int: column 0 = min, column 1 = max
  * Limits: 1 <= n_eig <= n_beam <= BB_MAX_BEAMS, n_ant >= 1, wavelength > 0; coordinate range as for
- * bb_synth_collect_eig. The call stages its inputs; the glue runs batched over up to 32 staged collects
- * (when 32 are staged, on bb_synth_flush, or on bb_synth_get) on the context's glue stream. */
+ * bb_synth_collect_eig. The call stages its inputs; the glue runs batched over up to 128 staged collects
+ * (when 128 are staged, on bb_synth_flush, or on bb_synth_get) on the context's glue stream. */
 int bb_synth_collect(bb_synth* s, int n_ant, int n_beam, int n_eig, double wavelength,
                      const bb_c32* W, int ldw, const bb_c32* S, int lds, const double* xyz,
                      int ldxyz, const double* intervals, int ld_int);
@@ -113,7 +113,7 @@ int bb_synth_collect_ex(bb_synth* s, int n_ant, int n_beam, int n_eig, double wa
 /* ---- collect_batch: Algorithm 1 for n_collects time steps / channels in one call (the
  * eigendecomposition is repeated for every time step and band). Same per-collect semantics as
  * bb_synth_collect (one LSQ filter, sinc Gram), applied in order c = 0 .. n_collects-1; the Gram matrices,
- * Cholesky factorisations and Hermitian eigensolves run as batched device calls (32 collects at a time); the
+ * Cholesky factorisations and Hermitian eigensolves run as batched device calls (up to 128 collects at a time); the
  * synthesizer of one group runs while the glue of the next is in progress.
  *   wavelengths  n_collects float64, HOST pointer
  *   S, xyz       collect c starts at S + c * stride_s, xyz + c * stride_xyz (strides in elements)

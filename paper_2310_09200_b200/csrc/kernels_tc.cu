@@ -52,7 +52,7 @@ constexpr int kK = 2 * kAC;             // K-columns (cos, sin per antenna) per 
 constexpr int kRec = 48;                // bytes of one antenna record {IH[3],0 | 2pi PH[3],0 | 2pi PL[3],0}
 constexpr int kMaxNE = 64;              // eigenpairs per slab
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t
+constexpr uint32_t kColD = 0;           // D of tile t at kColD + 128 t (+ 64 for the second buffer when N <= 64)
 constexpr int kLsTile = 512;            // bytes of one mini-GEMM B operand tile (16 antennas x 16 halves)
 constexpr float kTwoPi = 6.283185307179586f;
 
@@ -291,9 +291,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   uint64_t* b_empty = b_full + kSB;        // [kSB]
   uint64_t* a_full = b_empty + kSB;        // [kSA][2 tiles]
   uint64_t* a_empty = a_full + 2 * kSA;    // [kSA]
-  uint64_t* d_full = a_empty + kSA;
-  uint64_t* d_empty = d_full + 1;
-  uint64_t* ls_full = d_empty + 1;         // [kSA][2 tiles]
+  uint64_t* d_full = a_empty + kSA;        // [2 buffers]
+  uint64_t* d_empty = d_full + 2;          // [2 buffers]
+  uint64_t* ls_full = d_empty + 2;         // [kSA][2 tiles]
   uint64_t* apix_full = ls_full + 2 * kSA; // [2 tiles]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(apix_full + 2);
 
@@ -302,8 +302,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   if (tid == 0) {
     for (int s = 0; s < kSB; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 2); }      // 2: one commit per tile issuer
     for (int s = 0; s < kSA; ++s) { mbar_init(&a_full[2 * s], 4); mbar_init(&a_full[2 * s + 1], 4); mbar_init(&a_empty[s], 2); }
-    mbar_init(d_full, 2);
-    mbar_init(d_empty, kProducerWarps);
+    mbar_init(&d_full[0], 2); mbar_init(&d_full[1], 2);
+    mbar_init(&d_empty[0], kProducerWarps); mbar_init(&d_empty[1], kProducerWarps);
     for (int b = 0; b < 2 * kSA; ++b) mbar_init(&ls_full[b], 1);
     mbar_init(&apix_full[0], 4); mbar_init(&apix_full[1], 4);
     fence_barrier_init();
@@ -330,6 +330,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const int total = n_collects * n_chunks;
+  // N <= 64 accumulator columns per tile: the 128 columns of a tile hold TWO accumulators, so the MMAs of collect
+  // e + 1 run while the producers still read collect e (the epilogue is 8 % of a 20-collect launch otherwise)
+  const bool dbuf = N <= 64;
 
   if (warp < kProducerWarps) {
     // ===================== producers / epilogue: one pixel (TMEM lane) per thread =====================
@@ -423,7 +426,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         ++next_epi;
         next_due += n_chunks;
         const float* dcur = dsm + (size_t)(e & 1) * n_levels * NE;
-        mbar_wait(d_full, (uint32_t)(e & 1));
+        const int db = dbuf ? (e & 1) : 0;                   // accumulator buffer of collect e and the parity of its use
+        const uint32_t dph = dbuf ? (uint32_t)((e >> 1) & 1) : (uint32_t)(e & 1);
+        mbar_wait(&d_full[db], dph);
         tc_fence_after();
         named_bar_sync(1, kProducerWarps * 32);            // weights of collect e are in shared memory; buffer (e+1)&1 is free
         float wnext[4];                                    // prefetch the weights of collect e + 1 (<= 2048 floats)
@@ -432,7 +437,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           for (int u = 0; u < 4; ++u)
             if (woff[u] >= 0) wnext[u] = weights[(size_t)(e + 1) * weight_stride + woff[u]];
         }
-        const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128);
+        const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128 + db * 64);
         float2 pw[kMaxNE / 4];                             // |E|^2 of this group's eigenpair octets g = group, group + 2, ...
 #pragma unroll
         for (int gg = 0; gg < kMaxNE / 16; ++gg) {
@@ -454,7 +459,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(d_empty);               // D may be overwritten by the next collect
+        if (lane == 0) mbar_arrive(&d_empty[db]);          // this accumulator may be overwritten by a later collect
         for (int l = 0; l < n_levels; ++l) {               // a3: I_l += sum_k D[l,k] |E_k|^2 (packed pairs over k)
           float2 sacc = make_float2(0.f, 0.f);
 #pragma unroll
@@ -498,7 +503,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       const uint64_t desc0 = make_b_desc(smem_u32(stage_base), lbo, sbo);
       const uint32_t step16 = (2 * lbo) >> 4;              // one MMA consumes two 16-byte core columns of B
       const uint32_t chunk16 = chunk_bytes >> 4, half16 = half_bytes >> 4;
-      const uint32_t d = tb + kColD + t * 128;
+      const uint32_t d0 = tb + kColD + t * 128;
       int n = 0;
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
@@ -531,7 +536,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         if (total > 1) issue_mini();
       }
       for (int e = 0; e < n_collects; ++e) {
-        mbar_wait(d_empty, (uint32_t)((e & 1) ^ 1));
+        const int db = dbuf ? (e & 1) : 0;
+        const uint32_t d = d0 + (uint32_t)db * 64;
+        mbar_wait(&d_empty[db], (dbuf ? (uint32_t)((e >> 1) & 1) : (uint32_t)(e & 1)) ^ 1);
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
           if (C::kLsOnTensor) {
@@ -564,7 +571,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           }
           if (!C::kLsOnTensor) tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
-          if (c == n_chunks - 1) tc_commit(d_full);
+          if (c == n_chunks - 1) tc_commit(&d_full[db]);
           if (++sa == kSA) { sa = 0; pa ^= 1; }
           if (++sb == kSB) { sb = 0; pb ^= 1; }
         }
@@ -755,7 +762,7 @@ template <int MODE>
 int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) +                       2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 4) * 8 + 16 + 1024;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) +                       2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 6) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;

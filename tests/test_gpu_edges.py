@@ -84,14 +84,14 @@ def test_queue_overflow_additivity_reset_and_determinism(bb, ctx, oracle, varian
     ref = np.zeros((2, 400))
     s = bb.StandardSynthesis(ctx, c["pix"], 2, variant)
     cases = []
-    for e in range(70):             # more collects than the queue holds: several launches accumulate
+    for e in range(300):            # more collects than the queue holds (128): several launches accumulate
         B = np.asfortranarray((c["B"] * np.exp(1j * rng.uniform(0, 6.28, size=8))).astype(np.complex64))
         xyz = np.asfortranarray(c["xyz"] + rng.normal(0, 5.0, size=c["xyz"].shape))
         cases.append((B, xyz))
         oracle.synth(B, c["D"], xyz, c["pix"], c["wavelength"], img=ref)
         s.collect_eig(B, c["D"], xyz, c["wavelength"])
     a = s.images()
-    assert_parity(a, ref, "70 collects")
+    assert_parity(a, ref, "300 collects")
     s.reset()
     assert np.all(s.images() == 0)
     for B, xyz in cases:
@@ -251,12 +251,57 @@ def test_one_handle_many_shapes_and_staging_sizes(bb, ctx, oracle, variant):
     S1 = np.array([[2.5]], dtype=np.complex64)
     iv13 = np.asfortranarray(np.column_stack([np.arange(13.0), np.arange(13.0) + 1.0]))
     x1 = np.asfortranarray(np.array([[1.0, 2.0, 3.0]]))
-    for _ in range(40):                                        # more collects than queue slots
+    for _ in range(150):                                       # more collects than queue slots
         s13.collect(S1, None, x1, wl, 1, iv13)
     ref13 = np.zeros((13, 400))
-    for _ in range(40):
+    for _ in range(150):
         oracle.collect(S1, None, x1, wl, 1, iv13, pix, img=ref13)
     assert_parity(s13.images(), ref13, "%s 1x1" % variant)
+
+
+@pytest.mark.parametrize("kind", ["decaying", "flat", "indefinite", "wide_block", "clustered_cut"])
+def test_eigen_stage_on_every_kind_of_spectrum(bb, ctx, oracle, kind):
+    """The glue's leading-eigenpair solver (block subspace iteration, eig_subspace.cu) must either converge or hand
+    over to the full batched eigensolve; whichever path runs, eigenvalues and level images must match the oracle:
+    a decaying spectrum (the fast path's home ground), a flat one (no separation: fallback), an indefinite one (large
+    negative eigenvalues: powers of C would find those), a block wider than half the matrix (not applicable) and a
+    spectrum with a tight cluster right below the N_eig cut (slow convergence)."""
+    from paper_2310_09200_b200 import workloads
+    rng = np.random.default_rng({"decaying": 1, "flat": 2, "indefinite": 3, "wide_block": 4, "clustered_cut": 5}[kind])
+    n, wl = 288, 2.0
+    xyz = np.asfortranarray(np.column_stack([rng.uniform(-400, 400, size=(n, 2)), rng.normal(0, 2, n)]))
+    lm = rng.uniform(-0.08, 0.08, size=(300, 2))
+    pix = np.asfortranarray(np.column_stack([lm, np.sqrt(1 - np.sum(lm * lm, axis=1))]))
+    Q, _ = np.linalg.qr(rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n)))
+    n_eig = 24
+    if kind == "decaying":
+        ev = np.concatenate([10.0 ** np.linspace(3, 0, 60), np.full(n - 60, 0.3)])
+    elif kind == "flat":
+        ev = 1.0 + 1e-3 * rng.random(n)
+    elif kind == "indefinite":
+        ev = np.concatenate([10.0 ** np.linspace(2, 0, 40), np.full(n - 80, 0.1), -np.linspace(50, 500, 40)])
+    elif kind == "wide_block":
+        ev = np.concatenate([10.0 ** np.linspace(3, 0, 150), np.full(n - 150, 0.3)])
+        n_eig = 100
+    else:
+        ev = np.concatenate([10.0 ** np.linspace(3, 2, n_eig), 99.0 - 1e-3 * np.arange(80), np.full(n - n_eig - 80, 0.2)])
+    S = (Q * ev) @ Q.conj().T
+    S = np.asfortranarray((0.5 * (S + S.conj().T)).astype(np.complex64))
+    lam_ref, _ = oracle.eig_stage(S, None, xyz, wl, n_eig)
+    lam, _ = ctx.eig(S, None, xyz, wl, n_eig)
+    assert np.allclose(lam, lam_ref, rtol=1e-8, atol=1e-8 * np.abs(lam_ref).max()), (kind, np.max(np.abs(lam - lam_ref)))
+    if kind == "flat":
+        return                                  # level images of a (near-)degenerate spectrum are ill-conditioned (SURVEY 8c Q13): eigenvalues only
+    edges = [0.5 * (lam_ref[n_eig // 2 - 1] + lam_ref[n_eig // 2])]
+    iv = np.array([[edges[0], 1e30], [-1e30, edges[0]]])
+    ref = np.zeros((2, 300))
+    s = bb.StandardSynthesis(ctx, pix, 2, "fp32")
+    for _ in range(3):
+        oracle.collect(S, None, xyz, wl, n_eig, iv, pix, img=ref)
+        s.collect(S, None, xyz, wl, n_eig, iv)
+    got = s.images()
+    s.status()
+    assert_parity(got, ref, kind)
 
 
 def test_context_refuses_to_die_before_its_handles(bb):
