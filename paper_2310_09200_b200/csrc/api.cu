@@ -76,6 +76,8 @@ struct bb_synth {
   double rc[3] = {0, 0, 0};
   double rmax = 0;
   float* img = nullptr;
+  float* split_scratch = nullptr;              // tensor variants: partial level sums of a collect-range split launch
+  size_t split_cap = 0;                        // floats
   int* status_dev = nullptr;            // sticky BB_FLAG_* word
   int* status_pin = nullptr;
   cudaEvent_t ev_in = nullptr, ev_out = nullptr, ev_glue = nullptr;
@@ -228,6 +230,7 @@ extern "C" int bb_synth_destroy(bb_synth* s) {
   if (s->ev_glue) cudaEventDestroy(s->ev_glue);
   cudaFree(s->rprime);
   cudaFree(s->img);
+  cudaFree(s->split_scratch);
   cudaFree(s->status_dev);
   if (s->status_pin) cudaFreeHost(s->status_pin);
   cudaGetLastError();
@@ -308,6 +311,20 @@ static int launch_queue(bb_synth* s) {
   a.n_collects = s->q_len; a.n_levels = s->n_levels;
   a.img = s->img; a.img_stride = s->pix_stride;
   cudaStream_t st = s->ctx->synth_stream;
+  if (s->variant != BB_VARIANT_FP32) {
+    a.n_split = bb_tc_split(s->n_pix, s->q_len, s->ctx->sm_count);
+    if (a.n_split > 1) {
+      const size_t need = (size_t)a.n_split * s->n_levels * s->pix_stride;
+      if (need > s->split_cap) {                 // grows only; earlier launches that read it are complete once the stream is
+        BB_CUDA(cudaStreamSynchronize(st));
+        cudaFree(s->split_scratch);
+        s->split_scratch = nullptr; s->split_cap = 0;
+        if (cudaMalloc(&s->split_scratch, need * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+        s->split_cap = need;
+      }
+      a.scratch = s->split_scratch;
+    }
+  }
   int launches = 0, rc;
   {
     SpanGuard g(s, T_SYNTH, st);

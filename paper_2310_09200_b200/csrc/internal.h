@@ -86,7 +86,10 @@ struct SynthArgs {
   const float* weights; size_t weight_stride;              // floats per slot
   int n_collects, n_levels;
   float* img; int64_t img_stride;                          // [level][img_stride]
+  float* scratch; int n_split;                             // tensor variants: [n_split][level][img_stride] partial sums (NULL / 1: none)
 };
+// number of collect ranges a launch over n_collects is split into (1 = one CTA per pixel tile handles them all)
+int bb_tc_split(int64_t n_pix, int n_collects, int sm_count);
 // returns number of kernels launched in *launches
 int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);

@@ -30,14 +30,17 @@
 //   lo half of the A stage the producers fill next. The 32-bit fraction becomes a float by an integer add onto
 //   an exponent pattern (no I2F on the MUFU pipe), then one FFMA and MUFU.SIN/COS.
 //
-// CTA = 2 pixel tiles of 128 (256 pixels), 608 threads, 1 CTA per SM, all 512 TMEM columns:
-//   warps 0-15 producers + epilogue (two groups alternating chunks): phase generator, hi/lo split,
+// CTA = 2 pixel tiles of 128 (256 pixels), 1 CTA per SM, all 512 TMEM columns; G producer groups (FP16 modes: 3 groups,
+// 864 threads at 72 registers; TF32 mode: 2 groups, 608 threads):
+//   warps 0 .. 8G-1  producers + epilogue (groups take chunks in turn): phase generator, hi/lo split,
 //              tcgen05.st of their A rows straight into TMEM (A operand from TMEM: no smem round trip);
 //              per collect: tcgen05.ld of D, |E|^2, level weights, level sums.
-//   warps 16,17 one elected thread per pixel tile issues tcgen05.mma.cta_group::1 (A from TMEM, B from smem
-//              descriptors) and tcgen05.commit to the stage / accumulator mbarriers; warp 16 owns TMEM alloc.
-//   warp 18    one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
+//   warps 8G, 8G+1   one elected thread per pixel tile issues tcgen05.mma.cta_group::1 (A from TMEM, B from smem
+//              descriptors) and tcgen05.commit to the stage / accumulator mbarriers; warp 8G owns TMEM alloc.
+//   warp 8G+2  one elected thread streams the pre-tiled B chunks (UMMA canonical K-major no-swizzle
 //              layout, written by prep_tc_kernel) global -> shared with cp.async.bulk on mbarriers.
+// Small images: grid.y splits every tile's collects into ranges so that the CTA count fills whole waves of SMs
+// (bb_tc_split); the ranges' level sums are added in a fixed order by reduce_splits_kernel.
 #include "internal.h"
 #include <cuda_fp16.h>
 #include <cuda_fp8.h>
@@ -45,8 +48,6 @@
 namespace {
 
 constexpr int kTilePixels = 256;        // pixels per CTA (2 tiles of 128 TMEM lanes)
-constexpr int kProducerWarps = 16;      // 2 groups x 2 tiles x 4 lane quadrants
-constexpr int kThreadsTC = (kProducerWarps + 3) * 32;   // + one MMA issuer per tile + the loader
 constexpr int kAC = 16;                 // antennas per chunk
 constexpr int kK = 2 * kAC;             // K-columns (cos, sin per antenna) per chunk and pass
 constexpr int kRec = 48;                // bytes of one antenna record {IH[3],0 | 2pi PH[3],0 | 2pi PL[3],0}
@@ -59,6 +60,7 @@ constexpr float kTwoPi = 6.283185307179586f;
 template <int MODE> struct Cfg;
 template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (tile, hi|lo); small phase part on CUDA cores
   static constexpr int kElem = 4, kSA = 2, kSB = 4, kColsHalf = kK, kMmaPerPass = kK / 8;
+  static constexpr int kGroups = 2;     // producer groups taking chunks in turn
   static constexpr uint32_t kFmt = 2;   // instruction-descriptor operand format: TF32
   static constexpr bool kLsOnTensor = false;
   static constexpr uint32_t kColLs = 0;                  // unused
@@ -67,6 +69,7 @@ template <> struct Cfg<BB_TC_TF32> {    // 4-byte operands: 32 A columns per (ti
 };
 template <> struct Cfg<BB_TC_FP16> {    // 2-byte operands: (cos, sin) of one antenna share a 32-bit column
   static constexpr int kElem = 2, kSA = 3, kSB = 6, kColsHalf = kK / 2, kMmaPerPass = kK / 16;
+  static constexpr int kGroups = 3;     // one producer group per A stage
   static constexpr uint32_t kFmt = 0;   // F16
   static constexpr bool kLsOnTensor = true;              // small phase part as a K=16 mini-GEMM (see below)
   static constexpr uint32_t kColLs = 256;                // mini-GEMM A operand (per-pixel constants): 8 columns per tile
@@ -260,19 +263,36 @@ __device__ __forceinline__ void split_f16f8(float c, float s, uint32_t& hi, uint
 // Chunk in global/shared memory (N = 2 NE rows, kK columns of kElem bytes):
 //   [ B_hi : (kK*kElem/16) core columns x (N/8) row groups x (8 rows x 16 B) ][ B_lo : same ][ kAC antenna records ]
 //
-// Producer warps: w = 0..15; lane quadrant w & 3 (the TMEM lanes a warp may touch), tile (w >> 2) & 1,
-// group w >> 3. Group g produces the chunks n with (n & 1) == g, so each SM sub-partition always holds four
-// producer warps in different phases of their chunk (latency hiding) while per-chunk fixed costs stay
-// amortised over 16 antennas. The epilogue of collect e is deferred until both groups have produced their
-// first chunk of collect e+1, so the tensor pipe restarts on ready operands as soon as D is released;
-// the two groups split the eigenpair columns of D between them.
+// Producer warps: w = 0 .. 8 G - 1; lane quadrant w & 3 (the TMEM lanes a warp may touch), tile (w >> 2) & 1,
+// group w >> 3. Group g produces the chunks n = g, g + G, ..., so each SM sub-partition always holds producer
+// warps in different phases of their chunk (latency hiding) while per-chunk fixed costs stay amortised over
+// 16 antennas. The epilogue of collect e is deferred until a group has produced its first chunk of collect
+// e + 1, so the tensor pipe restarts on ready operands as soon as D is released; the groups split the eigenpair
+// columns of D between them.
+//
+// What paces the FP16 modes (per-warp clock64 traces) is a LOOP three chunks long, not a pipe: the A rows
+// of chunk n feed MMAs behind which the mini-GEMM of chunk n + 3 writes its ls into the same A stage, and that ls is
+// what the producers of chunk n + 3 need first. Hence: one producer group per A stage (a group never waits for
+// another group's stage), the mini-GEMM issued straight behind the MMAs that free its columns, and the operands of
+// chunk n + 3 waited for together with the A rows of chunk n.
 template <int MODE>
-__global__ void __launch_bounds__(kThreadsTC, 1)
+__global__ void __launch_bounds__((8 * Cfg<MODE>::kGroups + 3) * 32, 1)
 synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                 const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                 const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset, int NE,
-                int n_collects, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride) {
+                int n_collects_all, int n_chunks, int n_levels, float* __restrict__ img, int64_t img_stride,
+                int collects_per_split, float* __restrict__ scratch) {
   using C = Cfg<MODE>;
+  // gridDim.y > 1: this CTA handles the collects [e0, e0 + n_collects) of its pixel tile and leaves its level sums in
+  // scratch[blockIdx.y] (summed into the images, in a fixed order, by reduce_splits_kernel)
+  const int e0 = (int)blockIdx.y * collects_per_split;
+  const int n_collects = min(collects_per_split, n_collects_all - e0);
+  packed += (size_t)e0 * packed_stride;
+  weights += (size_t)e0 * weight_stride;
+  constexpr int kGroups = C::kGroups;
+  constexpr int kProducerWarps = 8 * kGroups;              // groups x 2 tiles x 4 lane quadrants
+  constexpr int kThreadsTC = (kProducerWarps + 3) * 32;    // + one MMA issuer per tile + the loader
+  constexpr int kOctPerGroup = (kMaxNE / 8 + kGroups - 1) / kGroups;   // eigenpair octets of D one group reduces
   constexpr int kSA = C::kSA, kSB = C::kSB;
   constexpr uint32_t kColA = C::kColA;
   constexpr uint32_t kColsStage = 4 * C::kColsHalf;                 // 2 tiles x (hi | lo)
@@ -285,7 +305,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
 
   unsigned char* stage_base = smem_raw;
   float* lev = reinterpret_cast<float*>(smem_raw + align_up((size_t)kSB * chunk_bytes, 1024));   // [2 groups][L][256]
-  float* dsm = lev + 2 * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
+  float* dsm = lev + kGroups * (size_t)n_levels * kTilePixels;                                         // [2][L][NE]
   uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + 2 * (size_t)n_levels * NE);
   uint64_t* b_full = bars;                 // [kSB]
   uint64_t* b_empty = b_full + kSB;        // [kSB]
@@ -312,7 +332,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
   }
-  for (int i = tid; i < 2 * n_levels * kTilePixels; i += kThreadsTC) lev[i] = 0.f;
+  for (int i = tid; i < kGroups * n_levels * kTilePixels; i += kThreadsTC) lev[i] = 0.f;
   for (int i = tid; i < n_levels * NE; i += kThreadsTC) {          // weights of collect 0
     const int l = i / NE, k = i - l * NE;
     dsm[i] = weights[(size_t)l * n_eig_pad + eig_offset + k];
@@ -367,9 +387,9 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       woff[u] = i < n_levels * NE ? l * n_eig_pad + eig_offset + k : -1;
     }
     int next_epi = 0, next_due = n_chunks;                 // epilogue e is due once this group produced a chunk of collect e + 1
-    int sa = group, sb = group;                            // this group's chunks: n = group, group + 2, ...
-    uint32_t pa = 0, pb = 0;                               // phase parities of the A / B stage rings
-    for (int n = group;; n += 2) {
+    int sa = group % kSA, sb = group % kSB;                // this group's chunks: n = group, group + kGroups, ...
+    uint32_t pa = (uint32_t)(group / kSA) & 1u, pb = 0;    // phase parities of the A / B stage rings
+    for (int n = group;; n += kGroups) {
       const bool have = n < total;
       if (have) {
         if constexpr (C::kLsOnTensor) {
@@ -398,28 +418,31 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
           }
         } else {
           // small phase part of this chunk (minus 2 pi): the mini-GEMM left it in the lo half of this A stage
-          float ls[16];
-          tmem_ld16(a_col + C::kColsHalf, ls);
-          tmem_wait_ld();
           const int4* ihrec = reinterpret_cast<const int4*>(stage_base + (size_t)sb * chunk_bytes + 2 * half_bytes + 2 * kLsTile);
-          uint32_t hi[16], lo[16];                         // 16 antennas -> 16 packed (cos, sin) columns
 #pragma unroll
-          for (int a = 0; a < 16; ++a) {
-            float cs, sn;
-            phase_cs_ls(ihrec[a], ls[a], q.jx, q.jy, q.jz, cs, sn);
-            if constexpr (MODE == BB_TC_F16F8) split_f16f8(cs, sn, hi[a], lo[a]);
-            else split_f16(cs, sn, hi[a], lo[a]);
+          for (int h = 0; h < 2; ++h) {                    // 8 antennas at a time (registers: three groups run at 72 per thread)
+            float ls[8];
+            tmem_ld8(a_col + C::kColsHalf + 8 * h, ls);
+            tmem_wait_ld();
+            uint32_t hi[8], lo[8];                         // 8 antennas -> 8 packed (cos, sin) columns
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+              float cs, sn;
+              phase_cs_ls(ihrec[8 * h + a], ls[a], q.jx, q.jy, q.jz, cs, sn);
+              if constexpr (MODE == BB_TC_F16F8) split_f16f8(cs, sn, hi[a], lo[a]);
+              else split_f16(cs, sn, hi[a], lo[a]);
+            }
+            tmem_st8(a_col + 8 * h, hi[0], hi[1], hi[2], hi[3], hi[4], hi[5], hi[6], hi[7]);
+            tmem_st8(a_col + C::kColsHalf + 8 * h, lo[0], lo[1], lo[2], lo[3], lo[4], lo[5], lo[6], lo[7]);
           }
-          tmem_st16(a_col, hi);
-          tmem_st16(a_col + C::kColsHalf, lo);
         }
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&a_full[2 * sa + tile]);
       }
-      sa += 2; if (sa >= kSA) { sa -= kSA; pa ^= 1; }
-      sb += 2; if (sb >= kSB) { sb -= kSB; pb ^= 1; }
+      sa += kGroups; while (sa >= kSA) { sa -= kSA; pa ^= 1; }
+      sb += kGroups; if (sb >= kSB) { sb -= kSB; pb ^= 1; }
       // ---- a3: deferred epilogues (collect e once this group had a go at collect e + 1, or at the end) ----
       while (next_epi < n_collects && (next_due <= n || !have)) {
         const int e = next_epi;
@@ -438,10 +461,10 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
             if (woff[u] >= 0) wnext[u] = weights[(size_t)(e + 1) * weight_stride + woff[u]];
         }
         const uint32_t d_col = tmem_base + lane_field + kColD + (uint32_t)(tile * 128 + db * 64);
-        float2 pw[kMaxNE / 4];                             // |E|^2 of this group's eigenpair octets g = group, group + 2, ...
+        float2 pw[kOctPerGroup * 4];                       // |E|^2 of this group's eigenpair octets g = group, group + kGroups, ...
 #pragma unroll
-        for (int gg = 0; gg < kMaxNE / 16; ++gg) {
-          const int g = 2 * gg + group;
+        for (int gg = 0; gg < kOctPerGroup; ++gg) {
+          const int g = kGroups * gg + group;
           if (g * 8 < NE) {
             float re[8], im[8];
             tmem_ld8(d_col + g * 8, re);
@@ -463,8 +486,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         for (int l = 0; l < n_levels; ++l) {               // a3: I_l += sum_k D[l,k] |E_k|^2 (packed pairs over k)
           float2 sacc = make_float2(0.f, 0.f);
 #pragma unroll
-          for (int gg = 0; gg < kMaxNE / 16; ++gg) {
-            const int g = 2 * gg + group;
+          for (int gg = 0; gg < kOctPerGroup; ++gg) {
+            const int g = kGroups * gg + group;
             if (g * 8 < NE) {
               const float4* dl = reinterpret_cast<const float4*>(dcur + (size_t)l * NE + g * 8);
               const float4 w0 = dl[0], w1 = dl[1];
@@ -485,10 +508,15 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       }
       if (!have) break;
     }
-    named_bar_sync(1, kProducerWarps * 32);                // both groups' level sums are complete
+    named_bar_sync(1, kProducerWarps * 32);                // all groups' level sums are complete
     if (ok && group == 0)
-      for (int l = 0; l < n_levels; ++l)
-        img[(size_t)l * img_stride + j] += lev[(size_t)l * kTilePixels + slot] + lev[(size_t)(n_levels + l) * kTilePixels + slot];
+      for (int l = 0; l < n_levels; ++l) {                 // fixed order: bit-identical run to run
+        float acc = lev[(size_t)l * kTilePixels + slot];
+#pragma unroll
+        for (int g = 1; g < kGroups; ++g) acc += lev[(size_t)(g * n_levels + l) * kTilePixels + slot];
+        if (gridDim.y > 1) scratch[((size_t)blockIdx.y * n_levels + l) * img_stride + j] = acc;
+        else img[(size_t)l * img_stride + j] += acc;
+      }
   } else if (warp < kProducerWarps + 2) {
     // ===================== MMA issuers: one warp per pixel tile =====================
     // One elected thread each; every operand is warp-uniform (the TMEM base is broadcast by shuffle and the
@@ -517,9 +545,11 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       const uint32_t a_pix = tb + C::kColLs + (uint32_t)t * 8;
       int sbm = 0, sam = 0;
       uint32_t pbm = 0;
-      auto issue_mini = [&]() {
-        mbar_wait(&b_full[sbm], pbm);
-        tc_fence_after();
+      auto issue_mini = [&](bool waited) {
+        if (!waited) {
+          mbar_wait(&b_full[sbm], pbm);
+          tc_fence_after();
+        }
         const uint64_t b1 = desc_ls0 + (uint64_t)((uint32_t)sbm * chunk16), b2 = b1 + (uint64_t)(kLsTile >> 4);
         const uint32_t dl = tb + kColA + (uint32_t)sam * kColsStage + (uint32_t)t * 2 * C::kColsHalf + C::kColsHalf;
         mma_ts<BB_TC_FP16>(dl, a_pix, b1, idesc_ls, 0u);   // A_hi B_hi + A_lo B_hi
@@ -528,12 +558,12 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         if (++sbm == kSB) { sbm = 0; pbm ^= 1; }
         if (++sam == kSA) sam = 0;
       };
+      constexpr int kLA = kSA;                             // chunks the mini-GEMM runs ahead of the main MMAs
       if (C::kLsOnTensor) {
-        static_assert(!C::kLsOnTensor || kSA >= 3, "the mini-GEMM runs two chunks ahead");
+        static_assert(!C::kLsOnTensor || (kSA >= 3 && kGroups <= kSA), "every group's first chunk of a collect has its ls before the accumulator hand-over");
         mbar_wait(&apix_full[t], 0);
         tc_fence_after();
-        if (total > 0) issue_mini();
-        if (total > 1) issue_mini();
+        for (int m = 0; m < kLA && m < total; ++m) issue_mini(false);
       }
       for (int e = 0; e < n_collects; ++e) {
         const int db = dbuf ? (e & 1) : 0;
@@ -541,9 +571,14 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
         mbar_wait(&d_empty[db], (dbuf ? (uint32_t)((e >> 1) & 1) : (uint32_t)(e & 1)) ^ 1);
         tc_fence_after();
         for (int c = 0; c < n_chunks; ++c, ++n) {
+          const bool more = n + kLA < total;
           if (C::kLsOnTensor) {
-            if (n + 2 < total) issue_mini();               // chunk n + 2 (its b_full wait covered chunk n two iterations ago)
-            mbar_wait(&a_full[2 * sa + t], pa);
+            if (more) {
+              // the operands of chunk n + kSA (normally long there: the B ring is kSB deep) and the A rows of chunk n
+              mbar_wait2(&b_full[sbm], pbm, &a_full[2 * sa + t], pa);
+            } else {
+              mbar_wait(&a_full[2 * sa + t], pa);
+            }
           } else {
             mbar_wait2(&b_full[sb], pb, &a_full[2 * sa + t], pa);
           }
@@ -569,6 +604,10 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
                 mma_ts<MODE>(d, a, bd, idesc, (c | pass | kk) != 0 ? 1u : 0u);
               }
           }
+          // chunk n + kSA's small phase part goes into the lo half of THIS A stage, straight behind the MMAs that read
+          // it (one thread's MMAs execute in order): the ls -> producers -> A rows -> ls loop, three chunks long, is
+          // what paces the kernel, so nothing else may sit between the two
+          if (C::kLsOnTensor && more) issue_mini(true);
           if (!C::kLsOnTensor) tc_commit(&a_empty[sa]);
           tc_commit(&b_empty[sb]);
           if (c == n_chunks - 1) tc_commit(&d_full[db]);
@@ -750,6 +789,17 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
     a.weights[(size_t)l * n_eig_pad + k] = (k < a.n_eig && in_range) ? a.D[l + (size_t)k * a.ldd] * wscale : 0.f;
 }
 
+// img[l][j] += sum over splits of scratch[s][l][j], splits in ascending order (deterministic)
+__global__ void reduce_splits_kernel(const float* __restrict__ scratch, int n_split, int n_levels, int64_t n_pix, int64_t stride,
+                                     float* __restrict__ img) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int l = blockIdx.y;
+  if (j >= n_pix) return;
+  float acc = img[(size_t)l * stride + j];
+  for (int s = 0; s < n_split; ++s) acc += scratch[((size_t)s * n_levels + l) * stride + j];
+  img[(size_t)l * stride + j] = acc;
+}
+
 template <int MODE>
 int launch_prep(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
   prep_tc_kernel<MODE><<<(unsigned)plan.n_eig_pad, 256, 0, st>>>(a, plan.eig_per_slab, plan.n_chunks, plan.n_eig_pad,
@@ -762,17 +812,26 @@ template <int MODE>
 int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* launches) {
   using C = Cfg<MODE>;
   const int NE = plan.eig_per_slab;
-  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) +                       2 * (size_t)a.n_levels * kTilePixels * 4 + 2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 6) * 8 + 16 + 1024;
+  constexpr int kThreadsTC = (8 * C::kGroups + 3) * 32;
+  const size_t smem = align_up((size_t)C::kSB * plan.chunk_bytes, 1024) + C::kGroups * (size_t)a.n_levels * kTilePixels * 4 +
+                      2 * (size_t)a.n_levels * NE * 4 + (2 * C::kSB + 5 * C::kSA + 6) * 8 + 16 + 1024;
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
+  const int n_split = a.scratch ? a.n_split : 1;
+  const int cps = (a.n_collects + n_split - 1) / n_split;
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
-    kern<<<(unsigned)tiles, kThreadsTC, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
-                                                   (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights, a.weight_stride,
-                                                   plan.n_eig_pad, slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img,
-                                                   a.img_stride);
+    kern<<<dim3((unsigned)tiles, (unsigned)n_split), kThreadsTC, smem, st>>>(
+        a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride, (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights,
+        a.weight_stride, plan.n_eig_pad, slab * NE, NE, a.n_collects, plan.n_chunks, a.n_levels, a.img, a.img_stride, cps, a.scratch);
     BB_CUDA(cudaGetLastError());
     ++*launches;
+    if (n_split > 1) {
+      reduce_splits_kernel<<<dim3((unsigned)((a.n_pix + 255) / 256), (unsigned)a.n_levels), 256, 0, st>>>(a.scratch, n_split, a.n_levels,
+                                                                                                     a.n_pix, a.img_stride, a.img);
+      BB_CUDA(cudaGetLastError());
+      ++*launches;
+    }
   }
   return BB_OK;
 }
@@ -796,6 +855,26 @@ TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels, int mode) {
   p.collect_bytes = (size_t)p.n_slabs * p.n_chunks * p.chunk_bytes;
   p.weight_floats = (size_t)n_levels * p.n_eig_pad;
   return p;
+}
+
+// Collect-range split for small images: the grid is one CTA per 256-pixel tile, so n_tiles / n_SM far from an integer
+// leaves SMs idle in the last wave (config 2: 256 tiles on 148 SMs = 1.73 waves). Splitting every tile's collects into
+// n_split ranges multiplies the CTA count; the smallest split (each range >= 4 collects) that lifts the wave efficiency
+// above 95 % is taken, or none if the unsplit grid is already within 5 % of the best.
+int bb_tc_split(int64_t n_pix, int n_collects, int sm_count) {
+  const int64_t tiles = (n_pix + kTilePixels - 1) / kTilePixels;
+  if (tiles <= 0 || sm_count <= 0) return 1;
+  auto eff = [&](int s) {
+    const int64_t ctas = tiles * s, waves = (ctas + sm_count - 1) / sm_count;
+    return (double)ctas / (double)(waves * sm_count);
+  };
+  int best = 1;
+  double best_eff = eff(1);
+  for (int s = 2; s <= 8 && n_collects / s >= 4; ++s) {
+    if (best_eff >= 0.95) break;
+    if (eff(s) > best_eff + 0.05) { best = s; best_eff = eff(s); }
+  }
+  return best;
 }
 
 int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
