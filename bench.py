@@ -255,15 +255,18 @@ def roofline_block(variant, flops_per_launch, avg_launch_ms, clocks, cfg_idx):
         r["frac_at_observed_clock"] = achieved / (peak * clocks["sm_mhz"] / SM_MAX_MHZ)
     # DRAM traffic of one launch: NOT measured in this run (that needs ncu) — the committed `ncu --set full` capture of
     # this command, labelled as such
-    for rnd in ("r02", "r01"):
+    for rnd in ("r02b", "r02", "r01"):
         prof = os.path.join(ROOT, "profiles", "%s_%s_ncu_full.csv" % (rnd, variant))
-        if cfg_idx == 4 and os.path.exists(prof):
+        if cfg_idx in (2, 3):
+            prof = os.path.join(ROOT, "profiles", "%s_%s_cfg%d_ncu_full.csv" % (rnd, variant, cfg_idx))
+        if cfg_idx in (2, 3, 4) and os.path.exists(prof):
             try:
                 import csv
-                mb = {row[0]: float(row[2]) for row in csv.reader(open(prof))
-                      if len(row) >= 3 and row[0].startswith("dram__bytes_") and row[1] == "Mbyte"}
+                scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+                mb = {row[0]: float(row[2]) * scale[row[1]] for row in csv.reader(open(prof))
+                      if len(row) >= 3 and row[0].startswith("dram__bytes_") and row[1] in scale}
                 if "dram__bytes_read.sum" in mb and "dram__bytes_write.sum" in mb:
-                    r["traffic"] = (mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]) * 1e6
+                    r["traffic"] = mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]
                     r["traffic_source"] = "committed ncu capture profiles/%s (not measured in this run)" % os.path.basename(prof)
                     break
             except Exception:
