@@ -209,6 +209,28 @@ int bb_estimate_n_eig(bb_ctx* ctx, const double* lambda, int n, double energy_fr
 int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int log_domain,
                      double* intervals_out, int ld_int);
 
+/* ---- NUFFT Synthesis (Section 2.5 Eq. 17-21, Section 3.4 Eq. 32-36, Algorithm 3), SURVEY 8(f) row 3 -----
+ * Per collect: V'_l = B diag(D[l,:]) B^H (Eq. 17 with the level selection of Eq. 21; Alg. 3 l.8) on the n_ant^2
+ * baselines b_pq = (x_p - x_q) / wavelength, then I_l(r_j) += sum_pq V'_l,pq exp(-2 pi i <b_pq, r_j>) (Eq. 18-19,
+ * DESIGN.md reading Q18) by a type-3 (nonuniform to nonuniform) 3-D NUFFT: centring and pre-phase, spreading with
+ * the "exponential of semicircle" kernel onto a fine grid (Eq. 33), a type-2 transform (deconvolve, zero-pad, FFT,
+ * interpolate: Eq. 34) and the diagonal correction by the kernel's Fourier transform (Eq. 35). The baselines and the
+ * pixels are partitioned into regular n_part_in x n_part_in x 1 and n_part_out x n_part_out x 1 cells along their two
+ * widest axes (Section 3.4.1, Eq. 36); every non-empty (input cell, output cell) pair is one transform.
+ * eps: requested relative tolerance (1e-2 .. 1e-7; sets the kernel width). pix as for bb_synth_create (host or
+ * device). B, D, xyz: host or device, as bb_synth_collect_eig; the call synchronises the context stream.
+ * BB_EUNSUPPORTED: a pair's fine grid would exceed 2^28 points: raise the partition counts.
+ * Same images as bb_synth_collect_eig up to eps; O(n_ant^2 L w^3 + grid log grid + n_pix L w^3) per pair. */
+typedef struct bb_nufft bb_nufft;
+int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pix, int n_levels, double eps,
+                    int n_part_in, int n_part_out, bb_nufft** out);
+int bb_nufft_destroy(bb_nufft* h);
+int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
+                         const float* D, int ldd, const double* xyz, int ldxyz);
+int bb_nufft_get(bb_nufft* h, int level, float* out);   /* n_pix floats, host or device; synchronises */
+/* number of transforms run and the largest fine grid (points) so far: what Section 3.4.1 / Figure 1c is about */
+int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_grid_points);
+
 const char* bb_status_string(int status);
 const char* bb_version(void);
 

@@ -28,7 +28,8 @@ _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_F
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
-           "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version"]
+           "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version",
+           "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
 
 _lib = None
 
@@ -75,6 +76,11 @@ def load_library(path: str = LIB_PATH):
         "bb_uvgrid_add": ([vp, i32, f64, vp, i32], i32),
         "bb_uvgrid_destroy": ([vp], i32),
         "bb_synth_set_weighting": ([vp, vp], i32),
+        "bb_nufft_create": ([vp, i64, vp, i64, i32, f64, i32, i32, pp], i32),
+        "bb_nufft_destroy": ([vp], i32),
+        "bb_nufft_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
+        "bb_nufft_get": ([vp, i32, vp], i32),
+        "bb_nufft_stats": ([vp, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)], i32),
         "bb_status_string": ([i32], ctypes.c_char_p),
         "bb_version": ([], ctypes.c_char_p),
     }
@@ -320,3 +326,44 @@ class StandardSynthesis:
 
     def launches(self) -> int:
         return int(_lib.bb_synth_launches(self._h))
+
+
+class NufftSynthesis:
+    """bb_nufft: NUFFT Synthesis (Section 3.4, Algorithm 3) — the same level images as StandardSynthesis.collect_eig up to
+    `eps`, through Gram-corrected visibilities per level and a partitioned 3-D type-3 NUFFT."""
+
+    def __init__(self, ctx: Context, pix, n_levels: int, eps: float = 1e-6, n_part_in: int = 1, n_part_out: int = 1):
+        keep = []
+        Pp, n_pix, c, ld = _marshal(pix, np.float64, keep)
+        assert c == 3, "pix must be (n_pix, 3)"
+        h = ctypes.c_void_p()
+        _check(_lib.bb_nufft_create(ctx._h, n_pix, Pp, ld, int(n_levels), float(eps), int(n_part_in), int(n_part_out),
+                                    ctypes.byref(h)), "bb_nufft_create")
+        self._h, self.ctx, self.n_pix, self.n_levels = h, ctx, n_pix, n_levels
+        import weakref
+        ctx._children.append(weakref.ref(self))
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.bb_nufft_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def collect_eig(self, B, D, xyz, wavelength):
+        keep = []
+        Bp, n_ant, n_eig, ldb = _marshal(B, np.complex64, keep)
+        Dp, _, _, ldd = _marshal(D, np.float32, keep)
+        Xp, _, _, ldx = _marshal(xyz, np.float64, keep)
+        _check(_lib.bb_nufft_collect_eig(self._h, n_ant, n_eig, float(wavelength), Bp, ldb, Dp, ldd, Xp, ldx), "bb_nufft_collect_eig")
+
+    def images(self):
+        out = np.empty((self.n_levels, self.n_pix), dtype=np.float32)
+        for l in range(self.n_levels):
+            _check(_lib.bb_nufft_get(self._h, l, out[l].ctypes.data), "bb_nufft_get")
+        return out
+
+    def stats(self):
+        a, b = ctypes.c_int64(), ctypes.c_int64()
+        _check(_lib.bb_nufft_stats(self._h, ctypes.byref(a), ctypes.byref(b)), "bb_nufft_stats")
+        return dict(n_transforms=a.value, max_grid_points=b.value)

@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 print(log)
     objs = [os.path.join(OBJ, f[:-3] + ".o") for f in srcs]
     if jobs or not os.path.exists(LIB):
-        cmd = [NVCC, "-shared", "-o", LIB] + objs + ["-L" + os.path.join(CUDA_HOME, "lib64"), "-lcusolver", "-lcublas",
+        cmd = [NVCC, "-shared", "-o", LIB] + objs + ["-L" + os.path.join(CUDA_HOME, "lib64"), "-lcusolver", "-lcublas", "-lcufft",
                                                      "-Xlinker", "-rpath," + os.path.join(CUDA_HOME, "lib64")]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:

@@ -107,6 +107,7 @@ struct bb_synth {
 cudaStream_t bb_ctx_glue_stream(bb_ctx* ctx) { return ctx->glue_stream; }
 cudaStream_t bb_ctx_user_stream(bb_ctx* ctx) { return ctx->stream; }
 int bb_ctx_device(bb_ctx* ctx) { return ctx->device; }
+void bb_ctx_ref(bb_ctx* ctx, int delta) { ctx->live_handles += delta; }   // handles of other translation units (bb_nufft)
 
 static bool is_device_ptr(const void* p) {
   cudaPointerAttributes at;

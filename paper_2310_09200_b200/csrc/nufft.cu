@@ -1,0 +1,455 @@
+// NUFFT Synthesis: Gram-corrected visibilities per level and a 3-D type-3 NUFFT with regular
+// domain partitioning of the baselines and the pixels (PAPER.md:129-164 Eq. 17-21; :345-423 Section 3.4, Eq. 32-36, Alg. 3).
+//
+//   I_l(r_j) += sum_n V_l,n exp(i <s_j, x_n>),   x_n = b_pq = (x_p - x_q) / lambda_w,   s_j = -2 pi r_j   (reading Q18)
+//
+// One transform = one (input cell, output cell) pair. With x = x_c + x', s = s_c + s' (cell centres):
+//   I_j = exp(i <s_j, x_c>) * F(s'_j),   F(s') = sum_n [V_n exp(i <s_c, x'_n>)] exp(i <s', x'_n>),   |x'_d| <= X_d, |s'_d| <= S_d.
+// Per dimension (upsampling sigma = 2, kernel width w, "exponential of semicircle" phi(z) = exp(beta (sqrt(1 - z^2) - 1))):
+//   1. spread (Eq. 33): grid of nf1 >= 2 sigma X S / pi + w points, source position x' sigma S / pi grid units from the middle;
+//   2. the grid values are Fourier coefficients g_m, m in [-nf1/2, nf1/2); F(s') = [sum_m g_m exp(i m theta)] / phihat(theta),
+//      theta = pi s' / (sigma S) in [-pi/sigma, pi/sigma]  (Eq. 34-35: phihat = the kernel's Fourier transform, by quadrature);
+//   3. the sum over m is a type-2 transform: divide g_m by phihat(2 pi m / nf2), zero-pad to nf2 >= sigma nf1, FFT (cuFFT),
+//      interpolate at theta with the same kernel.
+// Grids and FFTs are complex64; coordinates, phases and the kernel's transform are fp64. The host does the cell bookkeeping
+// (bounding boxes, index lists); everything that touches a visibility or a pixel value runs in the kernels below.
+#include "internal.h"
+#include <cufft.h>
+#include <algorithm>
+#include <cmath>
+#include <map>
+#include <new>
+#include <tuple>
+
+cudaStream_t bb_ctx_user_stream(bb_ctx* ctx);
+int bb_ctx_device(bb_ctx* ctx);
+void bb_ctx_ref(bb_ctx* ctx, int delta);
+
+namespace {
+
+constexpr int kMaxW = 12;               // kernel width (grid points) at most
+constexpr int kQuad = 32;               // Gauss-Legendre nodes on [0, 1] for the kernel's Fourier transform
+constexpr double kSigma = 2.0;          // upsampling of both stages
+constexpr int64_t kMaxGrid = (int64_t)1 << 28;
+
+__constant__ double c_gl_x[kQuad], c_gl_w[kQuad];
+
+struct KernelPar { int w; double beta; };
+
+__host__ __device__ inline double es_kernel(double z, double beta) {      // z = 2 t / w in [-1, 1]
+  const double a = 1.0 - z * z;
+  return a > 0.0 ? exp(beta * (sqrt(a) - 1.0)) : 0.0;
+}
+// phihat(k) = int_{-w/2}^{w/2} phi(2 t / w) exp(i k t) dt = w int_0^1 phi(z) cos(k w z / 2) dz      (k: radians per grid point)
+__device__ inline double es_hat_dev(double k, KernelPar kp) {
+  double acc = 0.0;
+  for (int q = 0; q < kQuad; ++q) acc += c_gl_w[q] * es_kernel(c_gl_x[q], kp.beta) * cos(0.5 * k * kp.w * c_gl_x[q]);
+  return acc * kp.w;
+}
+
+// Alg. 3 l.8 / Eq. 17, 21: V'_l[p, q] = sum_k D[l, k] B[p, k] conj(B[q, k]); out [l][p + n_ant q] complex64 (fp64 sums)
+__global__ void vis_kernel(const bb_c32* __restrict__ B, int ldb, const float* __restrict__ D, int ldd, int n_ant, int n_eig,
+                           int n_levels, float2* __restrict__ V) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (int64_t)n_ant * n_ant) return;
+  const int p = (int)(t % n_ant), q = (int)(t / n_ant);
+  for (int l = 0; l < n_levels; ++l) {
+    double re = 0.0, im = 0.0;
+    for (int k = 0; k < n_eig; ++k) {
+      const double d = D[l + (size_t)k * ldd];
+      if (d == 0.0) continue;
+      const bb_c32 a = B[p + (size_t)k * ldb], b = B[q + (size_t)k * ldb];
+      re += d * ((double)a.re * b.re + (double)a.im * b.im);
+      im += d * ((double)a.im * b.re - (double)a.re * b.im);
+    }
+    V[(size_t)l * n_ant * n_ant + t] = make_float2((float)re, (float)im);
+  }
+}
+
+struct CellGeom {                       // one (input cell, output cell) pair
+  double xc[3], sc[3];                  // centres of the sources (wavelengths) and of the targets' s = -2 pi r
+  double pos_scale[3];                  // grid units per unit of x': sigma S_d / pi
+  double theta_scale[3];                // theta per unit of s': pi / (sigma S_d)
+  int nf1[3], nf2[3];
+};
+
+// Eq. 33: spread the cell's sources onto the nf1 grid, all levels. idx: baseline ids (p + n_ant q) of the cell.
+__global__ void spread_kernel(const int* __restrict__ idx, int n_src, const double* __restrict__ xyz, int ldxyz, int n_ant,
+                              double inv_wl, const float2* __restrict__ V, int n_levels, CellGeom g, KernelPar kp,
+                              float2* __restrict__ grid) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_src) return;
+  const int id = idx[t], p = id % n_ant, q = id / n_ant;
+  double xp[3], ker[3][kMaxW];
+  int i0[3];
+  double ph = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    xp[d] = (xyz[p + (size_t)d * ldxyz] - xyz[q + (size_t)d * ldxyz]) * inv_wl - g.xc[d];
+    ph += g.sc[d] * xp[d];
+    const double pos = xp[d] * g.pos_scale[d] + 0.5 * g.nf1[d];          // grid units, well inside [w/2, nf1 - w/2]
+    i0[d] = (int)ceil(pos - 0.5 * kp.w);
+    for (int u = 0; u < kp.w; ++u) ker[d][u] = es_kernel(2.0 * (i0[d] + u - pos) / kp.w, kp.beta);
+  }
+  ph *= 0.15915494309189535;                                              // turns
+  ph -= rint(ph);
+  double sn, cs;
+  sincospi(2.0 * ph, &sn, &cs);
+  const size_t n1 = (size_t)g.nf1[0] * g.nf1[1] * g.nf1[2];
+  for (int l = 0; l < n_levels; ++l) {
+    const float2 v = V[(size_t)l * n_ant * n_ant + id];
+    const double cr = v.x * cs - v.y * sn, ci = v.x * sn + v.y * cs;      // V exp(i <s_c, x'>)
+    if (cr == 0.0 && ci == 0.0) continue;
+    float2* gl = grid + (size_t)l * n1;
+    for (int c = 0; c < kp.w; ++c)
+      for (int b = 0; b < kp.w; ++b) {
+        const double kzy = ker[2][c] * ker[1][b];
+        float2* row = gl + ((size_t)(i0[2] + c) * g.nf1[1] + (i0[1] + b)) * g.nf1[0] + i0[0];
+        for (int a = 0; a < kp.w; ++a) {
+          const double k3 = kzy * ker[0][a];
+          atomicAdd(&row[a].x, (float)(cr * k3));
+          atomicAdd(&row[a].y, (float)(ci * k3));
+        }
+      }
+  }
+}
+
+// type-2 step 1: fine[k] = g_m / (phihat2_x[mx] phihat2_y[my] phihat2_z[mz]) at k = m mod nf2 (FFT order); fine was zeroed.
+// dec: the three per-dimension arrays 1 / phihat(2 pi m / nf2), m = -nf1/2 .. nf1/2 - 1, concatenated.
+__global__ void deconv_pad_kernel(const float2* __restrict__ grid, int n_levels, CellGeom g, const double* __restrict__ dec,
+                                  float2* __restrict__ fine) {
+  const int64_t n1 = (int64_t)g.nf1[0] * g.nf1[1] * g.nf1[2];
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n1) return;
+  const int ix = (int)(t % g.nf1[0]), iy = (int)((t / g.nf1[0]) % g.nf1[1]), iz = (int)(t / ((int64_t)g.nf1[0] * g.nf1[1]));
+  const double f = dec[ix] * dec[g.nf1[0] + iy] * dec[g.nf1[0] + g.nf1[1] + iz];
+  const int kx = (ix - g.nf1[0] / 2 + g.nf2[0]) % g.nf2[0], ky = (iy - g.nf1[1] / 2 + g.nf2[1]) % g.nf2[1],
+            kz = (iz - g.nf1[2] / 2 + g.nf2[2]) % g.nf2[2];
+  const int64_t n2 = (int64_t)g.nf2[0] * g.nf2[1] * g.nf2[2];
+  const int64_t o = ((int64_t)kz * g.nf2[1] + ky) * g.nf2[0] + kx;
+  for (int l = 0; l < n_levels; ++l) {
+    const float2 v = grid[(size_t)l * n1 + t];
+    fine[(size_t)l * n2 + o] = make_float2((float)(v.x * f), (float)(v.y * f));
+  }
+}
+
+// Eq. 34-35: interpolate the FFT output at theta_j, divide by the spreading kernel's transform, apply the post-phase and
+// accumulate the real part into the level images. idx: pixel ids of the output cell.
+__global__ void interp_kernel(const int* __restrict__ idx, int n_tgt, const double* __restrict__ pix, int64_t ld_pix,
+                              const float2* __restrict__ fine, int n_levels, CellGeom g, KernelPar kp, float* __restrict__ img,
+                              int64_t img_stride) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_tgt) return;
+  const int j = idx[t];
+  double ker[3][kMaxW], corr = 1.0, post = 0.0;
+  int i0[3];
+  for (int d = 0; d < 3; ++d) {
+    const double s = -6.283185307179586 * pix[j + (size_t)d * ld_pix];
+    post += s * g.xc[d];
+    const double theta = (s - g.sc[d]) * g.theta_scale[d];
+    corr *= es_hat_dev(theta, kp);
+    const double pos = theta * g.nf2[d] * 0.15915494309189535;            // fine-grid units, may be negative: periodic
+    i0[d] = (int)ceil(pos - 0.5 * kp.w);
+    for (int u = 0; u < kp.w; ++u) ker[d][u] = es_kernel(2.0 * (i0[d] + u - pos) / kp.w, kp.beta);
+  }
+  post *= 0.15915494309189535;
+  post -= rint(post);
+  double sn, cs;
+  sincospi(2.0 * post, &sn, &cs);
+  const int64_t n2 = (int64_t)g.nf2[0] * g.nf2[1] * g.nf2[2];
+  for (int l = 0; l < n_levels; ++l) {
+    const float2* fl = fine + (size_t)l * n2;
+    double re = 0.0, im = 0.0;
+    for (int c = 0; c < kp.w; ++c) {
+      const int kz = ((i0[2] + c) % g.nf2[2] + g.nf2[2]) % g.nf2[2];
+      for (int b = 0; b < kp.w; ++b) {
+        const int ky = ((i0[1] + b) % g.nf2[1] + g.nf2[1]) % g.nf2[1];
+        const double kzy = ker[2][c] * ker[1][b];
+        const float2* row = fl + ((int64_t)kz * g.nf2[1] + ky) * g.nf2[0];
+        for (int a = 0; a < kp.w; ++a) {
+          const int kx = ((i0[0] + a) % g.nf2[0] + g.nf2[0]) % g.nf2[0];
+          const float2 v = row[kx];
+          const double k3 = kzy * ker[0][a];
+          re += k3 * v.x;
+          im += k3 * v.y;
+        }
+      }
+    }
+    img[(size_t)l * img_stride + j] += (float)((re * cs - im * sn) / corr);     // Re[ exp(i <s_j, x_c>) F / phihat ]
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------- host side
+struct bb_nufft {
+  bb_ctx* ctx = nullptr;
+  int64_t n_pix = 0, pix_stride = 0;
+  int n_levels = 0, n_part_in = 1, n_part_out = 1;
+  KernelPar kp{};
+  double* pix_dev = nullptr;            // [3][n_pix]
+  float* img = nullptr;                 // [level][pix_stride]
+  std::vector<double> pix_host;         // [3][n_pix]
+  // output cells (fixed per handle): pixel ids grouped by cell, bounding boxes
+  std::vector<int> out_start;           // n_cells + 1
+  int* out_idx_dev = nullptr;
+  std::vector<double> out_lo, out_hi;   // [cell][3]
+  // per-collect scratch (grown on demand)
+  float2 *V = nullptr, *grid = nullptr, *fine = nullptr;
+  size_t V_cap = 0, grid_cap = 0, fine_cap = 0;
+  int* in_idx_dev = nullptr; size_t in_idx_cap = 0;
+  double* dec_dev = nullptr; size_t dec_cap = 0;
+  bb_c32* B_dev = nullptr; float* D_dev = nullptr; double* xyz_dev = nullptr;
+  size_t B_cap = 0, D_cap = 0, xyz_cap = 0;
+  std::map<std::tuple<int, int, int>, cufftHandle> plans;
+  int64_t n_transforms = 0, max_grid = 0;
+};
+
+namespace {
+
+int next_smooth_even(int n) {           // smallest even 2^a 3^b 5^c >= n
+  if (n < 2) n = 2;
+  for (int m = n + (n & 1);; m += 2) {
+    int r = m;
+    while (r % 2 == 0) r /= 2;
+    while (r % 3 == 0) r /= 3;
+    while (r % 5 == 0) r /= 5;
+    if (r == 1) return m;
+  }
+}
+
+void gauss_legendre_01(double* x, double* w) {          // kQuad nodes and weights on [0, 1]
+  const int n = kQuad;
+  for (int i = 0; i < n; ++i) {
+    double z = cos(3.141592653589793 * (i + 0.75) / (n + 0.5)), pp = 1.0;
+    for (int it = 0; it < 100; ++it) {
+      double p1 = 1.0, p2 = 0.0;
+      for (int j = 0; j < n; ++j) { const double p3 = p2; p2 = p1; p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0); }
+      pp = n * (z * p1 - p2) / (z * z - 1.0);
+      const double dz = p1 / pp;
+      z -= dz;
+      if (fabs(dz) < 1e-15) break;
+    }
+    x[i] = 0.5 * (z + 1.0);
+    w[i] = 1.0 / ((1.0 - z * z) * pp * pp);              // (2 / ((1 - z^2) pp^2)) / 2: mapped to [0, 1]
+  }
+}
+
+double es_hat_host(double k, KernelPar kp, const double* x, const double* w) {
+  double acc = 0.0;
+  for (int q = 0; q < kQuad; ++q) acc += w[q] * es_kernel(x[q], kp.beta) * cos(0.5 * k * kp.w * x[q]);
+  return acc * kp.w;
+}
+
+template <class T>
+int grow(T** p, size_t* cap, size_t need) {
+  if (need <= *cap) return BB_OK;
+  cudaFree(*p);
+  *p = nullptr; *cap = 0;
+  if (cudaMalloc(p, need * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+  *cap = need;
+  return BB_OK;
+}
+
+// Regular partition of n points (coordinates c[d][i], d = 0..2) into parts x parts x 1 cells along the two widest axes:
+// cell id per point, then ids grouped by cell (counting sort) with each non-empty cell's bounding box.
+void partition(const double* c, int64_t n, int64_t ld, int parts, std::vector<int>& start, std::vector<int>& order,
+               std::vector<double>& lo, std::vector<double>& hi) {
+  double mn[3], mx[3];
+  for (int d = 0; d < 3; ++d) {
+    mn[d] = 1e300; mx[d] = -1e300;
+    for (int64_t i = 0; i < n; ++i) { mn[d] = std::min(mn[d], c[d * ld + i]); mx[d] = std::max(mx[d], c[d * ld + i]); }
+  }
+  int ax[3] = {0, 1, 2};
+  std::sort(ax, ax + 3, [&](int a, int b) { return mx[a] - mn[a] > mx[b] - mn[b]; });
+  const int n_cells = parts * parts;
+  std::vector<int> cell(n);
+  start.assign(n_cells + 1, 0);
+  for (int64_t i = 0; i < n; ++i) {
+    int id[2];
+    for (int u = 0; u < 2; ++u) {
+      const int d = ax[u];
+      const double ext = mx[d] - mn[d];
+      int k = ext > 0 ? (int)((c[d * ld + i] - mn[d]) / ext * parts) : 0;
+      id[u] = std::min(std::max(k, 0), parts - 1);
+    }
+    cell[i] = id[0] + parts * id[1];
+    start[cell[i] + 1] += 1;
+  }
+  for (int k = 0; k < n_cells; ++k) start[k + 1] += start[k];
+  order.resize(n);
+  std::vector<int> fill(start.begin(), start.end() - 1);
+  lo.assign((size_t)n_cells * 3, 1e300); hi.assign((size_t)n_cells * 3, -1e300);
+  for (int64_t i = 0; i < n; ++i) {
+    const int k = cell[i];
+    order[fill[k]++] = (int)i;
+    for (int d = 0; d < 3; ++d) { lo[k * 3 + d] = std::min(lo[k * 3 + d], c[d * ld + i]); hi[k * 3 + d] = std::max(hi[k * 3 + d], c[d * ld + i]); }
+  }
+}
+
+}  // namespace
+
+extern "C" int bb_nufft_destroy(bb_nufft* h) {
+  if (!h) return BB_OK;
+  cudaSetDevice(bb_ctx_device(h->ctx));
+  cudaStreamSynchronize(bb_ctx_user_stream(h->ctx));
+  for (auto& kv : h->plans) cufftDestroy(kv.second);
+  cudaFree(h->pix_dev); cudaFree(h->img); cudaFree(h->out_idx_dev); cudaFree(h->V); cudaFree(h->grid); cudaFree(h->fine);
+  cudaFree(h->in_idx_dev); cudaFree(h->dec_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
+  bb_ctx_ref(h->ctx, -1);
+  delete h;
+  return BB_OK;
+}
+
+extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pix, int n_levels, double eps,
+                               int n_part_in, int n_part_out, bb_nufft** out) {
+  if (!out) return BB_EINVAL;
+  *out = nullptr;
+  if (!ctx || n_pix < 1 || n_pix > 0x7fffffff || !pix || ld_pix < n_pix || n_levels < 1 || n_levels > BB_MAX_LEVELS ||
+      !(eps >= 1e-7 && eps <= 1e-2) || n_part_in < 1 || n_part_in > 64 || n_part_out < 1 || n_part_out > 64)
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(bb_ctx_device(ctx)));
+  bb_nufft* h = new (std::nothrow) bb_nufft;
+  if (!h) return BB_EALLOC;
+  h->ctx = ctx; h->n_pix = n_pix; h->pix_stride = (n_pix + 63) / 64 * 64; h->n_levels = n_levels;
+  bb_ctx_ref(ctx, +1);
+  h->n_part_in = n_part_in; h->n_part_out = n_part_out;
+  // kernel width from the tolerance (one more grid point per decade, as FINUFFT's rule for sigma = 2), beta = 2.30 w
+  h->kp.w = std::min(kMaxW, std::max(2, (int)ceil(-log10(eps / 10.0)) + 1));
+  h->kp.beta = 2.30 * h->kp.w;
+  double gx[kQuad], gw[kQuad];
+  gauss_legendre_01(gx, gw);
+  cudaStream_t st = bb_ctx_user_stream(ctx);
+  int rc = BB_OK;
+  do {
+    if (cudaMemcpyToSymbol(c_gl_x, gx, sizeof(gx)) != cudaSuccess || cudaMemcpyToSymbol(c_gl_w, gw, sizeof(gw)) != cudaSuccess) { rc = BB_ECUDA; break; }
+    h->pix_host.resize((size_t)3 * n_pix);
+    if (cudaStreamSynchronize(st) != cudaSuccess ||
+        cudaMemcpy2D(h->pix_host.data(), n_pix * sizeof(double), pix, ld_pix * sizeof(double), n_pix * sizeof(double), 3,
+                     cudaMemcpyDefault) != cudaSuccess) { rc = BB_ECUDA; break; }
+    if (cudaMalloc(&h->pix_dev, (size_t)3 * n_pix * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&h->img, (size_t)n_levels * h->pix_stride * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&h->out_idx_dev, (size_t)n_pix * sizeof(int)) != cudaSuccess) { rc = BB_EALLOC; break; }
+    std::vector<int> order;
+    partition(h->pix_host.data(), n_pix, n_pix, n_part_out, h->out_start, order, h->out_lo, h->out_hi);
+    if (cudaMemcpy(h->pix_dev, h->pix_host.data(), (size_t)3 * n_pix * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->out_idx_dev, order.data(), (size_t)n_pix * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemset(h->img, 0, (size_t)n_levels * h->pix_stride * sizeof(float)) != cudaSuccess) { rc = BB_ECUDA; break; }
+  } while (0);
+  if (rc != BB_OK) { cudaGetLastError(); bb_nufft_destroy(h); return rc; }
+  *out = h;
+  return BB_OK;
+}
+
+extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
+                                    const float* D, int ldd, const double* xyz, int ldxyz) {
+  if (!h || !B || !D || !xyz || n_ant < 1 || n_ant > 4096 || n_eig < 1 || n_eig > 4096 || !(wavelength > 0.0) || ldb < n_ant ||
+      ldd < h->n_levels || ldxyz < n_ant)
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
+  cudaStream_t st = bb_ctx_user_stream(h->ctx);
+  const int L = h->n_levels, w = h->kp.w;
+  const int64_t n_base = (int64_t)n_ant * n_ant;
+  int rc;
+  if ((rc = grow(&h->B_dev, &h->B_cap, (size_t)n_ant * n_eig)) != BB_OK || (rc = grow(&h->D_dev, &h->D_cap, (size_t)L * n_eig)) != BB_OK ||
+      (rc = grow(&h->xyz_dev, &h->xyz_cap, (size_t)3 * n_ant)) != BB_OK || (rc = grow(&h->V, &h->V_cap, (size_t)L * n_base)) != BB_OK ||
+      (rc = grow(&h->in_idx_dev, &h->in_idx_cap, (size_t)n_base)) != BB_OK)
+    return rc;
+  // snapshot the inputs (host or device: unified addressing), compact
+  BB_CUDA(cudaMemcpy2DAsync(h->B_dev, (size_t)n_ant * 8, B, (size_t)ldb * 8, (size_t)n_ant * 8, n_eig, cudaMemcpyDefault, st));
+  BB_CUDA(cudaMemcpy2DAsync(h->D_dev, (size_t)L * 4, D, (size_t)ldd * 4, (size_t)L * 4, n_eig, cudaMemcpyDefault, st));
+  BB_CUDA(cudaMemcpy2DAsync(h->xyz_dev, (size_t)n_ant * 8, xyz, (size_t)ldxyz * 8, (size_t)n_ant * 8, 3, cudaMemcpyDefault, st));
+  vis_kernel<<<(unsigned)((n_base + 255) / 256), 256, 0, st>>>(h->B_dev, n_ant, h->D_dev, L, n_ant, n_eig, L, h->V);
+  BB_CUDA(cudaGetLastError());
+  // baselines on the host for the cell bookkeeping (Section 3.4.1): coordinates only, no visibility values
+  std::vector<double> xh((size_t)3 * n_ant), bl((size_t)3 * n_base);
+  BB_CUDA(cudaMemcpyAsync(xh.data(), h->xyz_dev, xh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BB_CUDA(cudaStreamSynchronize(st));
+  for (int d = 0; d < 3; ++d)
+    for (int q = 0; q < n_ant; ++q)
+      for (int p = 0; p < n_ant; ++p) bl[(size_t)d * n_base + p + (size_t)n_ant * q] = (xh[(size_t)d * n_ant + p] - xh[(size_t)d * n_ant + q]) / wavelength;
+  std::vector<int> in_start, in_order;
+  std::vector<double> in_lo, in_hi;
+  partition(bl.data(), n_base, n_base, h->n_part_in, in_start, in_order, in_lo, in_hi);
+  BB_CUDA(cudaMemcpyAsync(h->in_idx_dev, in_order.data(), (size_t)n_base * sizeof(int), cudaMemcpyHostToDevice, st));
+  double gx[kQuad], gw[kQuad];
+  gauss_legendre_01(gx, gw);
+  const int n_in = h->n_part_in * h->n_part_in, n_out = h->n_part_out * h->n_part_out;
+  std::vector<double> dec;
+  for (int ic = 0; ic < n_in; ++ic) {
+    const int n_src = in_start[ic + 1] - in_start[ic];
+    if (n_src == 0) continue;
+    for (int oc = 0; oc < n_out; ++oc) {
+      const int n_tgt = h->out_start[oc + 1] - h->out_start[oc];
+      if (n_tgt == 0) continue;
+      CellGeom g{};
+      int64_t n1 = 1, n2 = 1;
+      for (int d = 0; d < 3; ++d) {
+        const double xl = in_lo[ic * 3 + d], xu = in_hi[ic * 3 + d];
+        const double sl = -6.283185307179586 * h->out_hi[oc * 3 + d], su = -6.283185307179586 * h->out_lo[oc * 3 + d];
+        g.xc[d] = 0.5 * (xl + xu); g.sc[d] = 0.5 * (sl + su);
+        const double X = std::max(0.5 * (xu - xl), 1e-9), S = std::max(0.5 * (su - sl), 1e-9);
+        // at least one grid point per unit of X S beyond the minimum, so that degenerate (thin) dimensions stay tiny
+        const double XS = std::max(X * S, 0.5);
+        const double S_eff = XS / X;                                  // S widened when X S is tiny: theta stays within +-pi/sigma
+        g.nf1[d] = next_smooth_even(std::max(2 * w, (int)ceil(2.0 * kSigma * X * S_eff / 3.141592653589793) + w + 2));
+        g.nf2[d] = next_smooth_even(std::max(2 * w, (int)ceil(kSigma * g.nf1[d])));
+        g.pos_scale[d] = kSigma * S_eff / 3.141592653589793;
+        g.theta_scale[d] = 3.141592653589793 / (kSigma * S_eff);
+        n1 *= g.nf1[d]; n2 *= g.nf2[d];
+      }
+      if (n2 > kMaxGrid) return BB_EUNSUPPORTED;
+      if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * n2)) != BB_OK ||
+          (rc = grow(&h->dec_dev, &h->dec_cap, (size_t)(g.nf1[0] + g.nf1[1] + g.nf1[2]))) != BB_OK)
+        return rc;
+      // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step)
+      dec.resize((size_t)(g.nf1[0] + g.nf1[1] + g.nf1[2]));
+      size_t o = 0;
+      for (int d = 0; d < 3; ++d)
+        for (int i = 0; i < g.nf1[d]; ++i) dec[o++] = 1.0 / es_hat_host(6.283185307179586 * (i - g.nf1[d] / 2) / g.nf2[d], h->kp, gx, gw);
+      BB_CUDA(cudaStreamSynchronize(st));                             // dec / plan reuse: the previous pair is done
+      BB_CUDA(cudaMemcpyAsync(h->dec_dev, dec.data(), dec.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+      BB_CUDA(cudaMemsetAsync(h->grid, 0, (size_t)L * n1 * sizeof(float2), st));
+      BB_CUDA(cudaMemsetAsync(h->fine, 0, (size_t)L * n2 * sizeof(float2), st));
+      spread_kernel<<<(unsigned)((n_src + 127) / 128), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_dev, n_ant, n_ant,
+                                                                    1.0 / wavelength, h->V, L, g, h->kp, h->grid);
+      BB_CUDA(cudaGetLastError());
+      deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, h->dec_dev, h->fine);
+      BB_CUDA(cudaGetLastError());
+      const auto key = std::make_tuple(g.nf2[0], g.nf2[1], g.nf2[2]);
+      auto it = h->plans.find(key);
+      if (it == h->plans.end()) {
+        cufftHandle plan;
+        int dims[3] = {g.nf2[2], g.nf2[1], g.nf2[0]};                 // slowest first
+        if (cufftPlanMany(&plan, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, 1) != CUFFT_SUCCESS) return BB_ECUDA;
+        it = h->plans.emplace(key, plan).first;
+      }
+      if (cufftSetStream(it->second, st) != CUFFT_SUCCESS) return BB_ECUDA;
+      for (int l = 0; l < L; ++l)                                      // u_k = sum_m b_m exp(+i m k h2): the unnormalised inverse
+        if (cufftExecC2C(it->second, reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2),
+                         reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2), CUFFT_INVERSE) != CUFFT_SUCCESS) return BB_ECUDA;
+      interp_kernel<<<(unsigned)((n_tgt + 127) / 128), 128, 0, st>>>(h->out_idx_dev + h->out_start[oc], n_tgt, h->pix_dev, h->n_pix,
+                                                                    h->fine, L, g, h->kp, h->img, h->pix_stride);
+      BB_CUDA(cudaGetLastError());
+      h->n_transforms += 1;
+      h->max_grid = std::max(h->max_grid, n2);
+    }
+  }
+  BB_CUDA(cudaStreamSynchronize(st));
+  return BB_OK;
+}
+
+extern "C" int bb_nufft_get(bb_nufft* h, int level, float* out) {
+  if (!h || !out || level < 0 || level >= h->n_levels) return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
+  cudaStream_t st = bb_ctx_user_stream(h->ctx);
+  BB_CUDA(cudaMemcpyAsync(out, h->img + (size_t)level * h->pix_stride, (size_t)h->n_pix * sizeof(float), cudaMemcpyDefault, st));
+  BB_CUDA(cudaStreamSynchronize(st));
+  return BB_OK;
+}
+
+extern "C" int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_grid_points) {
+  if (!h) return BB_EINVAL;
+  if (n_transforms) *n_transforms = h->n_transforms;
+  if (max_grid_points) *max_grid_points = h->max_grid;
+  return BB_OK;
+}

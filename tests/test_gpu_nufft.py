@@ -1,0 +1,106 @@
+"""NUFFT Synthesis on the device (bb_nufft_*, csrc/nufft.cu; Section 2.5 Eq. 17-21, Section 3.4 Eq. 32-36, Alg. 3)
+against the oracle's direct baseline-domain double sum (oracle.nufft_direct = Eq. 19 written out, pinned in
+tests/test_oracle_pins.py to Standard Synthesis and a hand-typed fringe). The NUFFT is an approximation to a requested
+tolerance eps: the gate is north_star's (rel-L2 <= 1e-4, max-abs <= 1e-3 x peak) at eps = 1e-6, and the error must follow eps."""
+import numpy as np
+import pytest
+
+from helpers import assert_parity, parity_numbers
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bb():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2310_09200_b200 import binding
+    binding.load_library()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(bb):
+    return bb.Context(0)
+
+
+def case(seed, n_ant, n_eig, n_levels, n_side, extent, fov, wavelength=2.0, flat=True):
+    rng = np.random.default_rng(seed)
+    B = ((rng.normal(size=(n_ant, n_eig)) + 1j * rng.normal(size=(n_ant, n_eig))) / np.sqrt(n_ant)).astype(np.complex64)
+    D = (rng.uniform(0.5, 3.0, size=(n_levels, n_eig)) * (rng.integers(0, n_levels, size=n_eig)[None, :] == np.arange(n_levels)[:, None]))
+    xyz = rng.uniform(-extent, extent, size=(n_ant, 3)) * np.array([1.0, 1.0, 0.02 if flat else 1.0]) + np.array([3.1e5, -2.2e5, 1.0e5])
+    g = (np.arange(n_side) - n_side / 2) * (2 * np.sin(fov / 2) / n_side)
+    l, m = np.meshgrid(g, g, indexing="xy")
+    l, m = l.ravel(), m.ravel()
+    c = np.array([0.2, -0.3, np.sqrt(1 - 0.13)])
+    e1 = np.cross(c, [0, 0, 1.0]); e1 /= np.linalg.norm(e1)
+    e2 = np.cross(c, e1)
+    pix = l[:, None] * e1 + m[:, None] * e2 + np.sqrt(1 - l * l - m * m)[:, None] * c
+    return dict(B=np.asfortranarray(B), D=np.asfortranarray(D.astype(np.float32)), xyz=np.asfortranarray(xyz),
+                pix=np.asfortranarray(pix), wavelength=wavelength)
+
+
+def test_config1_single_domain(bb, ctx, oracle):
+    """Config 1 (16 antennas in a 200 m disk, 32 x 32 pixels over 10 degrees): one transform, no partitioning."""
+    from paper_2310_09200_b200 import workloads
+    w = workloads.make_workload(1)
+    ci = w.collect_inputs(0)
+    lam, B = oracle.eig_stage(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig)
+    iv = workloads.choose_intervals(lam, w.cfg.n_levels)
+    D = oracle.level_weights(lam, iv)
+    pix = w.pixels()
+    ref, imag = oracle.nufft_direct(B.astype(np.complex64), D.astype(np.float32), ci["xyz"], pix, ci["wavelength"])
+    assert imag <= 1e-9 * np.max(np.abs(ref))
+    h = bb.NufftSynthesis(ctx, pix, w.cfg.n_levels, eps=1e-6)
+    h.collect_eig(B.astype(np.complex64), D.astype(np.float32), ci["xyz"], ci["wavelength"])
+    got = h.images()
+    assert h.stats()["n_transforms"] == 1
+    assert_parity(got, ref, "NUFFT synthesis config 1")
+    # and the same images as the Standard Synthesizer's hot path on the same inputs
+    s = bb.StandardSynthesis(ctx, pix, w.cfg.n_levels, "fp32")
+    s.collect_eig(B.astype(np.complex64), D.astype(np.float32), ci["xyz"], ci["wavelength"])
+    assert_parity(got, s.images().astype(np.float64), "NUFFT vs Standard Synthesis config 1")
+
+
+@pytest.mark.parametrize("parts", [(1, 1), (2, 1), (1, 3), (4, 2), (3, 5)])
+def test_domain_partitioning_gives_the_same_images(bb, ctx, oracle, parts):
+    """Eq. 36: splitting the baselines into I cells and the pixels into O cells changes the grids, not the sum.
+    40 antennas over +-600 wavelengths, 48 x 48 pixels over 12 degrees, 3 levels, two collects accumulated."""
+    c1 = case(11, 40, 9, 3, 48, 1200.0, np.deg2rad(12.0))
+    c2 = case(12, 40, 9, 3, 48, 1200.0, np.deg2rad(12.0))
+    ref = oracle.nufft_direct(c1["B"], c1["D"], c1["xyz"], c1["pix"], c1["wavelength"])[0]
+    ref = ref + oracle.nufft_direct(c2["B"], c2["D"], c2["xyz"], c1["pix"], c2["wavelength"])[0]
+    h = bb.NufftSynthesis(ctx, c1["pix"], 3, eps=1e-6, n_part_in=parts[0], n_part_out=parts[1])
+    h.collect_eig(c1["B"], c1["D"], c1["xyz"], c1["wavelength"])
+    h.collect_eig(c2["B"], c2["D"], c2["xyz"], c2["wavelength"])
+    st = h.stats()
+    assert 2 <= st["n_transforms"] <= 2 * (parts[0] * parts[1]) ** 2
+    assert_parity(h.images(), ref, "NUFFT synthesis, partition %s" % (parts,))
+
+
+def test_error_follows_the_requested_tolerance_and_grids_shrink_with_partitioning(bb, ctx, oracle):
+    c = case(21, 32, 6, 2, 40, 600.0, np.deg2rad(10.0), flat=False)        # a genuinely 3-D baseline cloud
+    ref = oracle.nufft_direct(c["B"], c["D"], c["xyz"], c["pix"], c["wavelength"])[0]
+    errs, grids = [], []
+    for eps, parts in ((1e-2, 2), (1e-4, 2), (1e-6, 2), (1e-6, 6)):
+        h = bb.NufftSynthesis(ctx, c["pix"], 2, eps=eps, n_part_in=parts, n_part_out=parts)
+        h.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+        errs.append(max(r for r, _ in parity_numbers(h.images(), ref)))
+        grids.append(h.stats()["max_grid_points"])
+        h.close()
+    assert errs[0] <= 5e-2 and errs[1] <= 5e-4 and errs[2] <= 2e-5 and errs[3] <= 2e-5, errs
+    assert errs[2] < errs[1] < errs[0], errs
+    assert grids[3] < grids[2] / 4, grids                                   # Section 3.4.1 / Figure 1c: smaller FFT grids
+
+
+def test_argument_validation_and_grid_limit(bb, ctx):
+    c = case(31, 8, 4, 2, 8, 100.0, np.deg2rad(5.0))
+    with pytest.raises(bb.BluebildError):
+        bb.NufftSynthesis(ctx, c["pix"], 2, eps=1e-9)
+    with pytest.raises(bb.BluebildError):
+        bb.NufftSynthesis(ctx, c["pix"], 0)
+    big = case(32, 8, 4, 2, 8, 4.0e5, np.deg2rad(40.0))                      # +-200 000 wavelengths over 40 degrees, one cell
+    h = bb.NufftSynthesis(ctx, big["pix"], 2, eps=1e-6)
+    with pytest.raises(bb.BluebildError) as e:
+        h.collect_eig(big["B"], big["D"], big["xyz"], big["wavelength"])
+    assert e.value.code == 7                                                # BB_EUNSUPPORTED: raise the partition counts
