@@ -114,14 +114,14 @@ __global__ void spread_kernel(const int* __restrict__ idx, int n_src, const doub
 }
 
 // type-2 step 1: fine[k] = g_m / (phihat2_x[mx] phihat2_y[my] phihat2_z[mz]) at k = m mod nf2 (FFT order); fine was zeroed.
-// dec: the three per-dimension arrays 1 / phihat(2 pi m / nf2), m = -nf1/2 .. nf1/2 - 1, concatenated.
-__global__ void deconv_pad_kernel(const float2* __restrict__ grid, int n_levels, CellGeom g, const double* __restrict__ dec,
-                                  float2* __restrict__ fine) {
+// dec_d: per-dimension arrays 1 / phihat(2 pi m / nf2_d), m = -nf1_d/2 .. nf1_d/2 - 1.
+__global__ void deconv_pad_kernel(const float2* __restrict__ grid, int n_levels, CellGeom g, const double* __restrict__ dec0,
+                                  const double* __restrict__ dec1, const double* __restrict__ dec2, float2* __restrict__ fine) {
   const int64_t n1 = (int64_t)g.nf1[0] * g.nf1[1] * g.nf1[2];
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n1) return;
   const int ix = (int)(t % g.nf1[0]), iy = (int)((t / g.nf1[0]) % g.nf1[1]), iz = (int)(t / ((int64_t)g.nf1[0] * g.nf1[1]));
-  const double f = dec[ix] * dec[g.nf1[0] + iy] * dec[g.nf1[0] + g.nf1[1] + iz];
+  const double f = dec0[ix] * dec1[iy] * dec2[iz];
   const int kx = (ix - g.nf1[0] / 2 + g.nf2[0]) % g.nf2[0], ky = (iy - g.nf1[1] / 2 + g.nf2[1]) % g.nf2[1],
             kz = (iz - g.nf1[2] / 2 + g.nf2[2]) % g.nf2[2];
   const int64_t n2 = (int64_t)g.nf2[0] * g.nf2[1] * g.nf2[2];
@@ -188,7 +188,10 @@ struct bb_nufft {
   KernelPar kp{};
   double* pix_dev = nullptr;            // [3][n_pix]
   float* img = nullptr;                 // [level][pix_stride]
-  std::vector<double> pix_host;         // [3][n_pix]
+  std::vector<double> pix_host;         // [3][n_pix], in the rotated frame
+  double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};   // rows = the frame (e_u, e_v, e_w): e_w = mean pixel direction. <b, r> is invariant under
+                                        // the rotation, and in this frame the pixels are thin along w (1 - cos(FoV / 2)), so
+                                        // the unpartitioned third axis of an (n, n, 1) partition costs few grid points
   // output cells (fixed per handle): pixel ids grouped by cell, bounding boxes
   std::vector<int> out_start;           // n_cells + 1
   int* out_idx_dev = nullptr;
@@ -197,7 +200,7 @@ struct bb_nufft {
   float2 *V = nullptr, *grid = nullptr, *fine = nullptr;
   size_t V_cap = 0, grid_cap = 0, fine_cap = 0;
   int* in_idx_dev = nullptr; size_t in_idx_cap = 0;
-  double* dec_dev = nullptr; size_t dec_cap = 0;
+  std::map<std::pair<int, int>, double*> dec;   // (nf1, nf2) -> device array of 1 / phihat(2 pi m / nf2), built once
   bb_c32* B_dev = nullptr; float* D_dev = nullptr; double* xyz_dev = nullptr;
   size_t B_cap = 0, D_cap = 0, xyz_cap = 0;
   std::map<std::tuple<int, int, int>, cufftHandle> plans;
@@ -293,8 +296,9 @@ extern "C" int bb_nufft_destroy(bb_nufft* h) {
   cudaSetDevice(bb_ctx_device(h->ctx));
   cudaStreamSynchronize(bb_ctx_user_stream(h->ctx));
   for (auto& kv : h->plans) cufftDestroy(kv.second);
+  for (auto& kv : h->dec) cudaFree(kv.second);
   cudaFree(h->pix_dev); cudaFree(h->img); cudaFree(h->out_idx_dev); cudaFree(h->V); cudaFree(h->grid); cudaFree(h->fine);
-  cudaFree(h->in_idx_dev); cudaFree(h->dec_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
+  cudaFree(h->in_idx_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
   bb_ctx_ref(h->ctx, -1);
   delete h;
   return BB_OK;
@@ -329,6 +333,29 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
     if (cudaMalloc(&h->pix_dev, (size_t)3 * n_pix * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&h->img, (size_t)n_levels * h->pix_stride * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&h->out_idx_dev, (size_t)n_pix * sizeof(int)) != cudaSuccess) { rc = BB_EALLOC; break; }
+    {   // rotate the pixels into (e_u, e_v, e_w)
+      double m[3] = {0, 0, 0};
+      for (int d = 0; d < 3; ++d) { for (int64_t i = 0; i < n_pix; ++i) m[d] += h->pix_host[(size_t)d * n_pix + i]; }
+      double nm = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+      if (nm > 1e-12 * (double)n_pix) {
+        double* R = h->R;
+        for (int d = 0; d < 3; ++d) R[6 + d] = m[d] / nm;
+        int k = 0;                                                    // the coordinate axis least aligned with e_w
+        for (int d = 1; d < 3; ++d) if (fabs(R[6 + d]) < fabs(R[6 + k])) k = d;
+        double a[3] = {0, 0, 0};
+        a[k] = 1.0;
+        const double dot = R[6 + k];
+        double u[3], un = 0;
+        for (int d = 0; d < 3; ++d) { u[d] = a[d] - dot * R[6 + d]; un += u[d] * u[d]; }
+        un = sqrt(un);
+        for (int d = 0; d < 3; ++d) R[d] = u[d] / un;
+        R[3] = R[7] * R[2] - R[8] * R[1]; R[4] = R[8] * R[0] - R[6] * R[2]; R[5] = R[6] * R[1] - R[7] * R[0];   // e_v = e_w x e_u
+      }
+      for (int64_t i = 0; i < n_pix; ++i) {
+        const double x = h->pix_host[i], y = h->pix_host[(size_t)n_pix + i], z = h->pix_host[(size_t)2 * n_pix + i];
+        for (int d = 0; d < 3; ++d) h->pix_host[(size_t)d * n_pix + i] = h->R[3 * d] * x + h->R[3 * d + 1] * y + h->R[3 * d + 2] * z;
+      }
+    }
     std::vector<int> order;
     partition(h->pix_host.data(), n_pix, n_pix, n_part_out, h->out_start, order, h->out_lo, h->out_hi);
     if (cudaMemcpy(h->pix_dev, h->pix_host.data(), (size_t)3 * n_pix * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -364,6 +391,11 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
   std::vector<double> xh((size_t)3 * n_ant), bl((size_t)3 * n_base);
   BB_CUDA(cudaMemcpyAsync(xh.data(), h->xyz_dev, xh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
   BB_CUDA(cudaStreamSynchronize(st));
+  for (int p = 0; p < n_ant; ++p) {                                   // antenna positions into the handle's rotated frame
+    const double x = xh[p], y = xh[(size_t)n_ant + p], z = xh[(size_t)2 * n_ant + p];
+    for (int d = 0; d < 3; ++d) xh[(size_t)d * n_ant + p] = h->R[3 * d] * x + h->R[3 * d + 1] * y + h->R[3 * d + 2] * z;
+  }
+  BB_CUDA(cudaMemcpyAsync(h->xyz_dev, xh.data(), xh.size() * sizeof(double), cudaMemcpyHostToDevice, st));
   for (int d = 0; d < 3; ++d)
     for (int q = 0; q < n_ant; ++q)
       for (int p = 0; p < n_ant; ++p) bl[(size_t)d * n_base + p + (size_t)n_ant * q] = (xh[(size_t)d * n_ant + p] - xh[(size_t)d * n_ant + q]) / wavelength;
@@ -398,22 +430,29 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
         n1 *= g.nf1[d]; n2 *= g.nf2[d];
       }
       if (n2 > kMaxGrid) return BB_EUNSUPPORTED;
-      if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * n2)) != BB_OK ||
-          (rc = grow(&h->dec_dev, &h->dec_cap, (size_t)(g.nf1[0] + g.nf1[1] + g.nf1[2]))) != BB_OK)
-        return rc;
-      // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step)
-      dec.resize((size_t)(g.nf1[0] + g.nf1[1] + g.nf1[2]));
-      size_t o = 0;
-      for (int d = 0; d < 3; ++d)
-        for (int i = 0; i < g.nf1[d]; ++i) dec[o++] = 1.0 / es_hat_host(6.283185307179586 * (i - g.nf1[d] / 2) / g.nf2[d], h->kp, gx, gw);
-      BB_CUDA(cudaStreamSynchronize(st));                             // dec / plan reuse: the previous pair is done
-      BB_CUDA(cudaMemcpyAsync(h->dec_dev, dec.data(), dec.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+      if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * n2)) != BB_OK)
+        return rc;                                                    // (cudaFree of a buffer in use waits for the device)
+      // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step): one device array per (nf1, nf2), kept
+      const double* decp[3];
+      for (int d = 0; d < 3; ++d) {
+        const auto dk = std::make_pair(g.nf1[d], g.nf2[d]);
+        auto di = h->dec.find(dk);
+        if (di == h->dec.end()) {
+          dec.resize((size_t)g.nf1[d]);
+          for (int i = 0; i < g.nf1[d]; ++i) dec[i] = 1.0 / es_hat_host(6.283185307179586 * (i - g.nf1[d] / 2) / g.nf2[d], h->kp, gx, gw);
+          double* dp = nullptr;
+          if (cudaMalloc(&dp, dec.size() * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+          BB_CUDA(cudaMemcpy(dp, dec.data(), dec.size() * sizeof(double), cudaMemcpyHostToDevice));
+          di = h->dec.emplace(dk, dp).first;
+        }
+        decp[d] = di->second;
+      }
       BB_CUDA(cudaMemsetAsync(h->grid, 0, (size_t)L * n1 * sizeof(float2), st));
       BB_CUDA(cudaMemsetAsync(h->fine, 0, (size_t)L * n2 * sizeof(float2), st));
       spread_kernel<<<(unsigned)((n_src + 127) / 128), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_dev, n_ant, n_ant,
                                                                     1.0 / wavelength, h->V, L, g, h->kp, h->grid);
       BB_CUDA(cudaGetLastError());
-      deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, h->dec_dev, h->fine);
+      deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, decp[0], decp[1], decp[2], h->fine);
       BB_CUDA(cudaGetLastError());
       const auto key = std::make_tuple(g.nf2[0], g.nf2[1], g.nf2[2]);
       auto it = h->plans.find(key);
