@@ -463,6 +463,23 @@ def run_ours(args):
             del di
         line["configs"] = cfgs
 
+    # ---- NUFFT Synthesis, informational: config 1's collect through both synthesizers ------
+    if not args.quick and world == 1:
+        w1, it1, _, _ = prepare_inputs(1, ctx, binding, workloads)
+        p1 = w1.pixels()
+        ss = binding.StandardSynthesis(ctx, p1, w1.cfg.n_levels, "fp32")
+        nu = binding.NufftSynthesis(ctx, p1, w1.cfg.n_levels, eps=1e-6)
+        for obj in (ss, nu):                                  # warm-up (cuFFT plan, allocations)
+            obj.collect_eig(it1[0]["B"], it1[0]["D"], it1[0]["xyz"], it1[0]["wavelength"])
+        ref1, got1 = ss.images().astype(np.float64), nu.images().astype(np.float64)
+        t0 = time.perf_counter()
+        nu.collect_eig(it1[0]["B"], it1[0]["D"], it1[0]["xyz"], it1[0]["wavelength"])
+        nufft_ms = 1e3 * (time.perf_counter() - t0)
+        line["nufft"] = {"workload": "config 1: %s, one collect, eps 1e-6, one transform" % w1.cfg.name, "ms_per_collect_wall": nufft_ms,
+                         "rel_l2_vs_standard_fp32": float(max(np.linalg.norm(got1[l] - ref1[l]) / np.linalg.norm(ref1[l])
+                                                              for l in range(w1.cfg.n_levels))), **nu.stats()}
+        nu.close(); ss.close()
+
     if world == 1 and not args.no_cpu_baseline:
         from oracle import bluebild_oracle as oracle      # cpu_baseline leg: the one place bench.py runs the oracle
         oracle.build()

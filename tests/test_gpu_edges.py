@@ -304,13 +304,15 @@ def test_eigen_stage_on_every_kind_of_spectrum(bb, ctx, oracle, kind):
     assert_parity(got, ref, kind)
 
 
+@pytest.mark.parametrize("n_eig", [12, 70])          # 70: two eigen-slabs, i.e. two split launches sharing the scratch
 @pytest.mark.parametrize("variant", ["tf32x3", "fp16x3", "fp16fp8"])
-def test_collect_range_split_of_small_images(bb, ctx, oracle, variant):
+def test_collect_range_split_of_small_images(bb, ctx, oracle, variant, n_eig):
     """150 pixel tiles on 148 SMs would run as two half-empty waves, so the tensor launch splits every tile's collects
     into ranges (csrc/kernels_tc.cu bb_tc_split) whose partial level sums are added in a fixed order. 9 collects give
     the uneven ranges 5 + 4; the last tile is ragged; a second, shorter launch (3 collects: no split) accumulates into
     the same images; everything must match the oracle's plain sum and be bit-identical run to run."""
-    n_ant, n_eig, n_levels, n_pix = 48, 12, 3, 150 * 256 - 37
+    n_ant, n_levels, n_pix = 48, 3, 150 * 256 - 37
+    n_slabs = (n_eig + 63) // 64
     cases = [random_case(7000 + t, n_ant, n_eig, n_levels, n_pix) for t in range(12)]
     pix = cases[0]["pix"]
     sub = np.unique(np.concatenate([np.arange(0, n_pix, 97), np.arange(n_pix - 300, n_pix)]))
@@ -324,11 +326,11 @@ def test_collect_range_split_of_small_images(bb, ctx, oracle, variant):
             s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
         s.flush()
         l0 = s.launches()
-        assert l0 == 9 + 2, l0                      # 9 prep kernels, one split synthesizer launch + its reduction
+        assert l0 == 9 + 2 * n_slabs, l0            # 9 prep kernels, per slab one split synthesizer launch + its reduction
         for c in cases[9:]:
             s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
         runs.append(s.images())
-        assert s.launches() == l0 + 3 + 1           # too few collects to split: the plain launch
+        assert s.launches() == l0 + 3 + n_slabs     # too few collects to split: the plain launch
         s.close()
     assert np.array_equal(runs[0], runs[1])
     assert_parity(runs[0][:, sub], ref, "collect-range split %s" % variant)
