@@ -76,7 +76,7 @@ struct bb_synth {
   double rc[3] = {0, 0, 0};
   double rmax = 0;
   float* img = nullptr;
-  float* split_scratch = nullptr;              // tensor variants: partial level sums of a collect-range split launch
+  float* split_scratch = nullptr;              // partial level sums of a collect-range split launch (small images)
   size_t split_cap = 0;                        // floats
   int* status_dev = nullptr;            // sticky BB_FLAG_* word
   int* status_pin = nullptr;
@@ -312,8 +312,9 @@ static int launch_queue(bb_synth* s) {
   a.n_collects = s->q_len; a.n_levels = s->n_levels;
   a.img = s->img; a.img_stride = s->pix_stride;
   cudaStream_t st = s->ctx->synth_stream;
-  if (s->variant != BB_VARIANT_FP32) {
-    a.n_split = bb_tc_split(s->n_pix, s->q_len, s->ctx->sm_count);
+  {
+    a.n_split = s->variant == BB_VARIANT_FP32 ? bb_fp32_split(s->fplan, s->n_pix, s->q_len, s->ctx->sm_count)
+                                             : bb_tc_split(s->n_pix, s->q_len, s->ctx->sm_count);
     if (a.n_split > 1) {
       const size_t need = (size_t)a.n_split * s->n_levels * s->pix_stride;
       if (need > s->split_cap) {                 // grows only; earlier launches that read it are complete once the stream is

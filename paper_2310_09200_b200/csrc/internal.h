@@ -86,10 +86,15 @@ struct SynthArgs {
   const float* weights; size_t weight_stride;              // floats per slot
   int n_collects, n_levels;
   float* img; int64_t img_stride;                          // [level][img_stride]
-  float* scratch; int n_split;                             // tensor variants: [n_split][level][img_stride] partial sums (NULL / 1: none)
+  float* scratch; int n_split;                             // [n_split][level][img_stride] partial sums of a collect-range split (NULL / 1: none)
 };
-// number of collect ranges a launch over n_collects is split into (1 = one CTA per pixel tile handles them all)
+// number of collect ranges a launch over n_collects is split into (1 = one CTA per pixel tile handles them all):
+// generic rule (tiles, resident CTA slots of the GPU), and per kernel family
+int bb_collect_split(int64_t tiles, int n_collects, int cta_slots);
 int bb_tc_split(int64_t n_pix, int n_collects, int sm_count);
+int bb_fp32_split(const Fp32Plan& plan, int64_t n_pix, int n_collects, int sm_count);
+// img[l][j] += sum_s scratch[s][l][j], s ascending (deterministic)
+int bb_launch_reduce_splits(const float* scratch, int n_split, int n_levels, int64_t n_pix, int64_t stride, float* img, cudaStream_t st);
 // returns number of kernels launched in *launches
 int bb_launch_synth_fp32(const Fp32Plan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);
 int bb_launch_synth_tc(const TcPlan& plan, const SynthArgs& a, int sm_count, cudaStream_t st, int* launches);

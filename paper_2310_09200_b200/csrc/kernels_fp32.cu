@@ -73,8 +73,14 @@ __global__ void __launch_bounds__(kThreads, MINB)
 synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_stride,
                   const unsigned char* __restrict__ packed, size_t packed_stride, size_t slab_offset,
                   const float* __restrict__ weights, size_t weight_stride, int n_eig_pad, int eig_offset,
-                  int n_collects, int n_chunks, int AC, int n_levels, float* __restrict__ img,
-                  int64_t img_stride) {
+                  int n_collects_all, int n_chunks, int AC, int n_levels, float* __restrict__ img,
+                  int64_t img_stride, int collects_per_split, float* __restrict__ scratch) {
+  // gridDim.y > 1: collect-range split of a small image (kernels_tc.cu bb_collect_split): this CTA handles the collects
+  // [e0, e0 + n_collects) and leaves its level sums in scratch[blockIdx.y]
+  const int e0 = (int)blockIdx.y * collects_per_split;
+  const int n_collects = min(collects_per_split, n_collects_all - e0);
+  packed += (size_t)e0 * packed_stride;
+  weights += (size_t)e0 * weight_stride;
   constexpr int TG = kThreads / GC;       // threads per eigen-group
   constexpr int NQ = KT / 2;              // eigen-pairs per thread
   constexpr int ROW4 = GC * NQ;           // float4 per antenna row in a chunk
@@ -204,7 +210,8 @@ synth_fp32_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_
       float v = 0.f;
 #pragma unroll
       for (int gg = 0; gg < GC; ++gg) v += lev[((size_t)l * PT + p) * kThreads + gg * TG + tt];
-      img[(size_t)l * img_stride + j] += v;
+      if (gridDim.y > 1) scratch[((size_t)blockIdx.y * n_levels + l) * img_stride + j] = v;
+      else img[(size_t)l * img_stride + j] += v;
     }
   }
 }
@@ -295,13 +302,20 @@ int launch_variant(const Fp32Plan& plan, const SynthArgs& a, cudaStream_t st, in
   auto kern = synth_fp32_kernel<KT, PT, GC, MINB>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + TG * PT - 1) / (TG * PT);
+  const int n_split = a.scratch ? a.n_split : 1;
+  const int cps = (a.n_collects + n_split - 1) / n_split;
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
-    kern<<<(unsigned)tiles, kThreads, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
+    kern<<<dim3((unsigned)tiles, (unsigned)n_split), kThreads, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
                                                    (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights,
                                                    a.weight_stride, plan.n_eig_pad, slab * GC * KT, a.n_collects,
-                                                   plan.n_chunks, plan.AC, a.n_levels, a.img, a.img_stride);
+                                                   plan.n_chunks, plan.AC, a.n_levels, a.img, a.img_stride, cps, a.scratch);
     BB_CUDA(cudaGetLastError());
     ++*launches;
+    if (n_split > 1) {
+      const int rc = bb_launch_reduce_splits(a.scratch, n_split, a.n_levels, a.n_pix, a.img_stride, a.img, st);
+      if (rc != BB_OK) return rc;
+      ++*launches;
+    }
   }
   return BB_OK;
 }
@@ -327,6 +341,11 @@ Fp32Plan bb_fp32_plan(int n_ant, int n_eig, int n_levels) {
   p.collect_bytes = (size_t)p.n_slabs * p.n_chunks * p.chunk_bytes;
   p.weight_floats = (size_t)n_levels * p.n_eig_pad;
   return p;
+}
+
+int bb_fp32_split(const Fp32Plan& plan, int64_t n_pix, int n_collects, int sm_count) {
+  const int tile = (kThreads / plan.GC) * plan.PT;                   // pixels per CTA; MINB CTAs are resident per SM
+  return bb_collect_split((n_pix + tile - 1) / tile, n_collects, sm_count * plan.MINB);
 }
 
 int bb_launch_prep_fp32(const Fp32Plan& plan, const PrepArgs& a, cudaStream_t st) {

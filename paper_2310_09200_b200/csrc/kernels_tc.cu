@@ -827,9 +827,8 @@ int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* laun
     BB_CUDA(cudaGetLastError());
     ++*launches;
     if (n_split > 1) {
-      reduce_splits_kernel<<<dim3((unsigned)((a.n_pix + 255) / 256), (unsigned)a.n_levels), 256, 0, st>>>(a.scratch, n_split, a.n_levels,
-                                                                                                     a.n_pix, a.img_stride, a.img);
-      BB_CUDA(cudaGetLastError());
+      const int rc = bb_launch_reduce_splits(a.scratch, n_split, a.n_levels, a.n_pix, a.img_stride, a.img, st);
+      if (rc != BB_OK) return rc;
       ++*launches;
     }
   }
@@ -857,16 +856,15 @@ TcPlan bb_tc_plan(int n_ant, int n_eig, int n_levels, int mode) {
   return p;
 }
 
-// Collect-range split for small images: the grid is one CTA per 256-pixel tile, so n_tiles / n_SM far from an integer
-// leaves SMs idle in the last wave (config 2: 256 tiles on 148 SMs = 1.73 waves). Splitting every tile's collects into
+// Collect-range split for small images: the grid is one CTA per pixel tile, so n_tiles / (resident CTA slots) far from an
+// integer leaves SMs idle in the last wave (config 2, tensor variants: 256 tiles on 148 SMs = 1.73 waves). Splitting every tile's collects into
 // n_split ranges multiplies the CTA count; the smallest split (each range >= 4 collects) that lifts the wave efficiency
 // above 95 % is taken, or none if the unsplit grid is already within 5 % of the best.
-int bb_tc_split(int64_t n_pix, int n_collects, int sm_count) {
-  const int64_t tiles = (n_pix + kTilePixels - 1) / kTilePixels;
-  if (tiles <= 0 || sm_count <= 0) return 1;
+int bb_collect_split(int64_t tiles, int n_collects, int cta_slots) {
+  if (tiles <= 0 || cta_slots <= 0) return 1;
   auto eff = [&](int s) {
-    const int64_t ctas = tiles * s, waves = (ctas + sm_count - 1) / sm_count;
-    return (double)ctas / (double)(waves * sm_count);
+    const int64_t ctas = tiles * s, waves = (ctas + cta_slots - 1) / cta_slots;
+    return (double)ctas / (double)(waves * cta_slots);
   };
   int best = 1;
   double best_eff = eff(1);
@@ -875,6 +873,14 @@ int bb_tc_split(int64_t n_pix, int n_collects, int sm_count) {
     if (eff(s) > best_eff + 0.05) { best = s; best_eff = eff(s); }
   }
   return best;
+}
+int bb_tc_split(int64_t n_pix, int n_collects, int sm_count) {      // tensor variants: 256-pixel tiles, one CTA per SM
+  return bb_collect_split((n_pix + kTilePixels - 1) / kTilePixels, n_collects, sm_count);
+}
+int bb_launch_reduce_splits(const float* scratch, int n_split, int n_levels, int64_t n_pix, int64_t stride, float* img, cudaStream_t st) {
+  reduce_splits_kernel<<<dim3((unsigned)((n_pix + 255) / 256), (unsigned)n_levels), 256, 0, st>>>(scratch, n_split, n_levels, n_pix, stride, img);
+  BB_CUDA(cudaGetLastError());
+  return BB_OK;
 }
 
 int bb_launch_prep_tc(const TcPlan& plan, const PrepArgs& a, cudaStream_t st) {
