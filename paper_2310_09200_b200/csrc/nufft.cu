@@ -73,43 +73,44 @@ struct CellGeom {                       // one (input cell, output cell) pair
   int nf1[3], nf2[3];
 };
 
-// Eq. 33: spread the cell's sources onto the nf1 grid, all levels. idx: baseline ids (p + n_ant q) of the cell.
+// Eq. 33: spread the cell's sources onto the nf1 grid, all levels: one warp per source, the w^3 taps spread over the lanes.
+// idx: baseline ids (p + n_ant q) of the cell.
 __global__ void spread_kernel(const int* __restrict__ idx, int n_src, const double* __restrict__ xyz, int ldxyz, int n_ant,
                               double inv_wl, const float2* __restrict__ V, int n_levels, CellGeom g, KernelPar kp,
                               float2* __restrict__ grid) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= n_src) return;
+  __shared__ float ker_s[4][3][kMaxW];
+  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 4 + wib;
+  if (t >= n_src) return;                                                 // whole warps leave together
   const int id = idx[t], p = id % n_ant, q = id / n_ant;
-  double xp[3], ker[3][kMaxW];
   int i0[3];
   double ph = 0.0;
   for (int d = 0; d < 3; ++d) {
-    xp[d] = (xyz[p + (size_t)d * ldxyz] - xyz[q + (size_t)d * ldxyz]) * inv_wl - g.xc[d];
-    ph += g.sc[d] * xp[d];
-    const double pos = xp[d] * g.pos_scale[d] + 0.5 * g.nf1[d];          // grid units, well inside [w/2, nf1 - w/2]
+    const double xp = (xyz[p + (size_t)d * ldxyz] - xyz[q + (size_t)d * ldxyz]) * inv_wl - g.xc[d];
+    ph += g.sc[d] * xp;
+    const double pos = xp * g.pos_scale[d] + 0.5 * g.nf1[d];              // grid units, well inside [w/2, nf1 - w/2]
     i0[d] = (int)ceil(pos - 0.5 * kp.w);
-    for (int u = 0; u < kp.w; ++u) ker[d][u] = es_kernel(2.0 * (i0[d] + u - pos) / kp.w, kp.beta);
+    if (lane < kp.w) ker_s[wib][d][lane] = (float)es_kernel(2.0 * (i0[d] + lane - pos) / kp.w, kp.beta);
   }
+  __syncwarp();
   ph *= 0.15915494309189535;                                              // turns
   ph -= rint(ph);
   double sn, cs;
   sincospi(2.0 * ph, &sn, &cs);
   const size_t n1 = (size_t)g.nf1[0] * g.nf1[1] * g.nf1[2];
+  const int w = kp.w, w3 = w * w * w;
   for (int l = 0; l < n_levels; ++l) {
     const float2 v = V[(size_t)l * n_ant * n_ant + id];
-    const double cr = v.x * cs - v.y * sn, ci = v.x * sn + v.y * cs;      // V exp(i <s_c, x'>)
-    if (cr == 0.0 && ci == 0.0) continue;
+    const float cr = (float)(v.x * cs - v.y * sn), ci = (float)(v.x * sn + v.y * cs);      // V exp(i <s_c, x'>)
+    if (cr == 0.f && ci == 0.f) continue;
     float2* gl = grid + (size_t)l * n1;
-    for (int c = 0; c < kp.w; ++c)
-      for (int b = 0; b < kp.w; ++b) {
-        const double kzy = ker[2][c] * ker[1][b];
-        float2* row = gl + ((size_t)(i0[2] + c) * g.nf1[1] + (i0[1] + b)) * g.nf1[0] + i0[0];
-        for (int a = 0; a < kp.w; ++a) {
-          const double k3 = kzy * ker[0][a];
-          atomicAdd(&row[a].x, (float)(cr * k3));
-          atomicAdd(&row[a].y, (float)(ci * k3));
-        }
-      }
+    for (int tap = lane; tap < w3; tap += 32) {
+      const int a = tap % w, b = (tap / w) % w, c = tap / (w * w);
+      const float k3 = ker_s[wib][0][a] * ker_s[wib][1][b] * ker_s[wib][2][c];
+      float2* dst = gl + ((size_t)(i0[2] + c) * g.nf1[1] + (i0[1] + b)) * g.nf1[0] + i0[0] + a;
+      atomicAdd(&dst->x, cr * k3);
+      atomicAdd(&dst->y, ci * k3);
+    }
   }
 }
 
@@ -133,48 +134,51 @@ __global__ void deconv_pad_kernel(const float2* __restrict__ grid, int n_levels,
 }
 
 // Eq. 34-35: interpolate the FFT output at theta_j, divide by the spreading kernel's transform, apply the post-phase and
-// accumulate the real part into the level images. idx: pixel ids of the output cell.
+// accumulate the real part into the level images: one warp per pixel — lane q evaluates quadrature node q of the kernel's
+// transform (kQuad = 32) and the w^3 taps are spread over the lanes. idx: pixel ids of the output cell.
 __global__ void interp_kernel(const int* __restrict__ idx, int n_tgt, const double* __restrict__ pix, int64_t ld_pix,
                               const float2* __restrict__ fine, int n_levels, CellGeom g, KernelPar kp, float* __restrict__ img,
                               int64_t img_stride) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  static_assert(kQuad == 32, "one quadrature node per lane");
+  __shared__ float ker_s[4][3][kMaxW];
+  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 4 + wib;
   if (t >= n_tgt) return;
   const int j = idx[t];
-  double ker[3][kMaxW], corr = 1.0, post = 0.0;
+  double corr = 1.0, post = 0.0;
   int i0[3];
   for (int d = 0; d < 3; ++d) {
     const double s = -6.283185307179586 * pix[j + (size_t)d * ld_pix];
     post += s * g.xc[d];
     const double theta = (s - g.sc[d]) * g.theta_scale[d];
-    corr *= es_hat_dev(theta, kp);
+    double hq = c_gl_w[lane] * es_kernel(c_gl_x[lane], kp.beta) * cos(0.5 * theta * kp.w * c_gl_x[lane]);
+    for (int o = 16; o > 0; o >>= 1) hq += __shfl_xor_sync(0xffffffffu, hq, o);
+    corr *= hq * kp.w;                                                    // phihat(theta_d)
     const double pos = theta * g.nf2[d] * 0.15915494309189535;            // fine-grid units, may be negative: periodic
     i0[d] = (int)ceil(pos - 0.5 * kp.w);
-    for (int u = 0; u < kp.w; ++u) ker[d][u] = es_kernel(2.0 * (i0[d] + u - pos) / kp.w, kp.beta);
+    if (lane < kp.w) ker_s[wib][d][lane] = (float)es_kernel(2.0 * (i0[d] + lane - pos) / kp.w, kp.beta);
   }
+  __syncwarp();
   post *= 0.15915494309189535;
   post -= rint(post);
   double sn, cs;
   sincospi(2.0 * post, &sn, &cs);
   const int64_t n2 = (int64_t)g.nf2[0] * g.nf2[1] * g.nf2[2];
+  const int w = kp.w, w3 = w * w * w;
   for (int l = 0; l < n_levels; ++l) {
     const float2* fl = fine + (size_t)l * n2;
-    double re = 0.0, im = 0.0;
-    for (int c = 0; c < kp.w; ++c) {
-      const int kz = ((i0[2] + c) % g.nf2[2] + g.nf2[2]) % g.nf2[2];
-      for (int b = 0; b < kp.w; ++b) {
-        const int ky = ((i0[1] + b) % g.nf2[1] + g.nf2[1]) % g.nf2[1];
-        const double kzy = ker[2][c] * ker[1][b];
-        const float2* row = fl + ((int64_t)kz * g.nf2[1] + ky) * g.nf2[0];
-        for (int a = 0; a < kp.w; ++a) {
-          const int kx = ((i0[0] + a) % g.nf2[0] + g.nf2[0]) % g.nf2[0];
-          const float2 v = row[kx];
-          const double k3 = kzy * ker[0][a];
-          re += k3 * v.x;
-          im += k3 * v.y;
-        }
-      }
+    float re = 0.f, im = 0.f;
+    for (int tap = lane; tap < w3; tap += 32) {
+      const int a = tap % w, b = (tap / w) % w, c = tap / (w * w);
+      const int kx = ((i0[0] + a) % g.nf2[0] + g.nf2[0]) % g.nf2[0], ky = ((i0[1] + b) % g.nf2[1] + g.nf2[1]) % g.nf2[1],
+                kz = ((i0[2] + c) % g.nf2[2] + g.nf2[2]) % g.nf2[2];
+      const float2 v = fl[((int64_t)kz * g.nf2[1] + ky) * g.nf2[0] + kx];
+      const float k3 = ker_s[wib][0][a] * ker_s[wib][1][b] * ker_s[wib][2][c];
+      re += k3 * v.x;
+      im += k3 * v.y;
     }
-    img[(size_t)l * img_stride + j] += (float)((re * cs - im * sn) / corr);     // Re[ exp(i <s_j, x_c>) F / phihat ]
+    for (int o = 16; o > 0; o >>= 1) { re += __shfl_xor_sync(0xffffffffu, re, o); im += __shfl_xor_sync(0xffffffffu, im, o); }
+    if (lane == 0) img[(size_t)l * img_stride + j] += (float)(((double)re * cs - (double)im * sn) / corr);   // Re[e^{i<s_j,x_c>} F / phihat]
   }
 }
 
@@ -449,7 +453,7 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
       }
       BB_CUDA(cudaMemsetAsync(h->grid, 0, (size_t)L * n1 * sizeof(float2), st));
       BB_CUDA(cudaMemsetAsync(h->fine, 0, (size_t)L * n2 * sizeof(float2), st));
-      spread_kernel<<<(unsigned)((n_src + 127) / 128), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_dev, n_ant, n_ant,
+      spread_kernel<<<(unsigned)((n_src + 3) / 4), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_dev, n_ant, n_ant,
                                                                     1.0 / wavelength, h->V, L, g, h->kp, h->grid);
       BB_CUDA(cudaGetLastError());
       deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, decp[0], decp[1], decp[2], h->fine);
@@ -466,7 +470,7 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
       for (int l = 0; l < L; ++l)                                      // u_k = sum_m b_m exp(+i m k h2): the unnormalised inverse
         if (cufftExecC2C(it->second, reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2),
                          reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2), CUFFT_INVERSE) != CUFFT_SUCCESS) return BB_ECUDA;
-      interp_kernel<<<(unsigned)((n_tgt + 127) / 128), 128, 0, st>>>(h->out_idx_dev + h->out_start[oc], n_tgt, h->pix_dev, h->n_pix,
+      interp_kernel<<<(unsigned)((n_tgt + 3) / 4), 128, 0, st>>>(h->out_idx_dev + h->out_start[oc], n_tgt, h->pix_dev, h->n_pix,
                                                                     h->fine, L, g, h->kp, h->img, h->pix_stride);
       BB_CUDA(cudaGetLastError());
       h->n_transforms += 1;
