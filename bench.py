@@ -474,8 +474,9 @@ def run_ours(args):
         ref1, got1 = ss.images().astype(np.float64), nu.images().astype(np.float64)
         t0 = time.perf_counter()
         nu.collect_eig(it1[0]["B"], it1[0]["D"], it1[0]["xyz"], it1[0]["wavelength"])
+        nu.images()                                           # the transforms of the staged collect run here
         nufft_ms = 1e3 * (time.perf_counter() - t0)
-        line["nufft"] = {"workload": "config 1: %s, one collect, eps 1e-6, one transform" % w1.cfg.name, "ms_per_collect_wall": nufft_ms,
+        line["nufft"] = {"workload": "config 1: %s, one collect, eps 1e-6, one transform" % w1.cfg.name, "ms_per_collect_and_get_wall": nufft_ms,
                          "rel_l2_vs_standard_fp32": float(max(np.linalg.norm(got1[l] - ref1[l]) / np.linalg.norm(ref1[l])
                                                               for l in range(w1.cfg.n_levels))), **nu.stats()}
         nu.close(); ss.close()

@@ -75,18 +75,22 @@ struct CellGeom {                       // one (input cell, output cell) pair
 
 // Eq. 33: spread the cell's sources onto the nf1 grid, all levels: one warp per source, the w^3 taps spread over the lanes.
 // idx: baseline ids (p + n_ant q) of the cell.
-__global__ void spread_kernel(const int* __restrict__ idx, int n_src, const double* __restrict__ xyz, int ldxyz, int n_ant,
-                              double inv_wl, const float2* __restrict__ V, int n_levels, CellGeom g, KernelPar kp,
+// Source id = collect * n_ant^2 + p + n_ant q; xyz: [collect][3][n_ant] (rotated frame), inv_wl: [collect], V: [collect][level][n_ant^2].
+__global__ void spread_kernel(const int* __restrict__ idx, int n_src, const double* __restrict__ xyz, int n_ant,
+                              const double* __restrict__ inv_wl, const float2* __restrict__ V, int n_levels, CellGeom g, KernelPar kp,
                               float2* __restrict__ grid) {
   __shared__ float ker_s[4][3][kMaxW];
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = blockIdx.x * 4 + wib;
   if (t >= n_src) return;                                                 // whole warps leave together
-  const int id = idx[t], p = id % n_ant, q = id / n_ant;
+  const int n_base = n_ant * n_ant;
+  const int id = idx[t], col = id / n_base, bq = id - col * n_base, p = bq % n_ant, q = bq / n_ant;
+  const double* xc = xyz + (size_t)col * 3 * n_ant;
+  const double iw = inv_wl[col];
   int i0[3];
   double ph = 0.0;
   for (int d = 0; d < 3; ++d) {
-    const double xp = (xyz[p + (size_t)d * ldxyz] - xyz[q + (size_t)d * ldxyz]) * inv_wl - g.xc[d];
+    const double xp = (xc[p + (size_t)d * n_ant] - xc[q + (size_t)d * n_ant]) * iw - g.xc[d];
     ph += g.sc[d] * xp;
     const double pos = xp * g.pos_scale[d] + 0.5 * g.nf1[d];              // grid units, well inside [w/2, nf1 - w/2]
     i0[d] = (int)ceil(pos - 0.5 * kp.w);
@@ -100,7 +104,7 @@ __global__ void spread_kernel(const int* __restrict__ idx, int n_src, const doub
   const size_t n1 = (size_t)g.nf1[0] * g.nf1[1] * g.nf1[2];
   const int w = kp.w, w3 = w * w * w;
   for (int l = 0; l < n_levels; ++l) {
-    const float2 v = V[(size_t)l * n_ant * n_ant + id];
+    const float2 v = V[((size_t)col * n_levels + l) * n_base + bq];
     const float cr = (float)(v.x * cs - v.y * sn), ci = (float)(v.x * sn + v.y * cs);      // V exp(i <s_c, x'>)
     if (cr == 0.f && ci == 0.f) continue;
     float2* gl = grid + (size_t)l * n1;
@@ -207,6 +211,12 @@ struct bb_nufft {
   std::map<std::pair<int, int>, double*> dec;   // (nf1, nf2) -> device array of 1 / phihat(2 pi m / nf2), built once
   bb_c32* B_dev = nullptr; float* D_dev = nullptr; double* xyz_dev = nullptr;
   size_t B_cap = 0, D_cap = 0, xyz_cap = 0;
+  // staged collects: their visibilities wait in V ([collect][level][n_ant^2]) until bb_nufft_get (or the source cap) runs ONE set
+  // of transforms over the baselines of all of them — the paper's use of the NUFFT over all time steps
+  int pend = 0, pend_n_ant = 0;
+  std::vector<double> xyz_all, inv_wl_all;      // host: rotated antenna positions [collect][3][n_ant], 1 / wavelength
+  double* xyz_all_dev = nullptr; double* inv_wl_dev = nullptr;
+  size_t xyz_all_cap = 0, inv_wl_cap = 0;
   std::map<std::tuple<int, int, int>, cufftHandle> plans;
   int64_t n_transforms = 0, max_grid = 0;
 };
@@ -302,7 +312,7 @@ extern "C" int bb_nufft_destroy(bb_nufft* h) {
   for (auto& kv : h->plans) cufftDestroy(kv.second);
   for (auto& kv : h->dec) cudaFree(kv.second);
   cudaFree(h->pix_dev); cudaFree(h->img); cudaFree(h->out_idx_dev); cudaFree(h->V); cudaFree(h->grid); cudaFree(h->fine);
-  cudaFree(h->in_idx_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
+  cudaFree(h->in_idx_dev); cudaFree(h->xyz_all_dev); cudaFree(h->inv_wl_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
   bb_ctx_ref(h->ctx, -1);
   delete h;
   return BB_OK;
@@ -371,42 +381,35 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
   return BB_OK;
 }
 
-extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
-                                    const float* D, int ldd, const double* xyz, int ldxyz) {
-  if (!h || !B || !D || !xyz || n_ant < 1 || n_ant > 4096 || n_eig < 1 || n_eig > 4096 || !(wavelength > 0.0) || ldb < n_ant ||
-      ldd < h->n_levels || ldxyz < n_ant)
-    return BB_EINVAL;
-  BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
+constexpr int64_t kMaxPendingSources = (int64_t)1 << 25;
+
+// One set of transforms over the baselines of all staged collects (Eq. 36 over cells; the sum over time steps is just more sources).
+static int nufft_flush(bb_nufft* h) {
+  if (h->pend == 0) return BB_OK;
   cudaStream_t st = bb_ctx_user_stream(h->ctx);
-  const int L = h->n_levels, w = h->kp.w;
-  const int64_t n_base = (int64_t)n_ant * n_ant;
+  const int L = h->n_levels, w = h->kp.w, n_ant = h->pend_n_ant, T = h->pend;
+  const int64_t n_base = (int64_t)n_ant * n_ant, n_total = n_base * T;
   int rc;
-  if ((rc = grow(&h->B_dev, &h->B_cap, (size_t)n_ant * n_eig)) != BB_OK || (rc = grow(&h->D_dev, &h->D_cap, (size_t)L * n_eig)) != BB_OK ||
-      (rc = grow(&h->xyz_dev, &h->xyz_cap, (size_t)3 * n_ant)) != BB_OK || (rc = grow(&h->V, &h->V_cap, (size_t)L * n_base)) != BB_OK ||
-      (rc = grow(&h->in_idx_dev, &h->in_idx_cap, (size_t)n_base)) != BB_OK)
+  if ((rc = grow(&h->in_idx_dev, &h->in_idx_cap, (size_t)n_total)) != BB_OK || (rc = grow(&h->xyz_all_dev, &h->xyz_all_cap, h->xyz_all.size())) != BB_OK ||
+      (rc = grow(&h->inv_wl_dev, &h->inv_wl_cap, h->inv_wl_all.size())) != BB_OK)
     return rc;
-  // snapshot the inputs (host or device: unified addressing), compact
-  BB_CUDA(cudaMemcpy2DAsync(h->B_dev, (size_t)n_ant * 8, B, (size_t)ldb * 8, (size_t)n_ant * 8, n_eig, cudaMemcpyDefault, st));
-  BB_CUDA(cudaMemcpy2DAsync(h->D_dev, (size_t)L * 4, D, (size_t)ldd * 4, (size_t)L * 4, n_eig, cudaMemcpyDefault, st));
-  BB_CUDA(cudaMemcpy2DAsync(h->xyz_dev, (size_t)n_ant * 8, xyz, (size_t)ldxyz * 8, (size_t)n_ant * 8, 3, cudaMemcpyDefault, st));
-  vis_kernel<<<(unsigned)((n_base + 255) / 256), 256, 0, st>>>(h->B_dev, n_ant, h->D_dev, L, n_ant, n_eig, L, h->V);
-  BB_CUDA(cudaGetLastError());
+  BB_CUDA(cudaMemcpyAsync(h->xyz_all_dev, h->xyz_all.data(), h->xyz_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  BB_CUDA(cudaMemcpyAsync(h->inv_wl_dev, h->inv_wl_all.data(), h->inv_wl_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
   // baselines on the host for the cell bookkeeping (Section 3.4.1): coordinates only, no visibility values
-  std::vector<double> xh((size_t)3 * n_ant), bl((size_t)3 * n_base);
-  BB_CUDA(cudaMemcpyAsync(xh.data(), h->xyz_dev, xh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
-  BB_CUDA(cudaStreamSynchronize(st));
-  for (int p = 0; p < n_ant; ++p) {                                   // antenna positions into the handle's rotated frame
-    const double x = xh[p], y = xh[(size_t)n_ant + p], z = xh[(size_t)2 * n_ant + p];
-    for (int d = 0; d < 3; ++d) xh[(size_t)d * n_ant + p] = h->R[3 * d] * x + h->R[3 * d + 1] * y + h->R[3 * d + 2] * z;
+  std::vector<double> bl((size_t)3 * n_total);
+  for (int c = 0; c < T; ++c) {
+    const double* xh = h->xyz_all.data() + (size_t)c * 3 * n_ant;
+    const double iw = h->inv_wl_all[c];
+    for (int d = 0; d < 3; ++d)
+      for (int q = 0; q < n_ant; ++q)
+        for (int p = 0; p < n_ant; ++p)
+          bl[(size_t)d * n_total + (size_t)c * n_base + p + (size_t)n_ant * q] = (xh[(size_t)d * n_ant + p] - xh[(size_t)d * n_ant + q]) * iw;
   }
-  BB_CUDA(cudaMemcpyAsync(h->xyz_dev, xh.data(), xh.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-  for (int d = 0; d < 3; ++d)
-    for (int q = 0; q < n_ant; ++q)
-      for (int p = 0; p < n_ant; ++p) bl[(size_t)d * n_base + p + (size_t)n_ant * q] = (xh[(size_t)d * n_ant + p] - xh[(size_t)d * n_ant + q]) / wavelength;
   std::vector<int> in_start, in_order;
   std::vector<double> in_lo, in_hi;
-  partition(bl.data(), n_base, n_base, h->n_part_in, in_start, in_order, in_lo, in_hi);
-  BB_CUDA(cudaMemcpyAsync(h->in_idx_dev, in_order.data(), (size_t)n_base * sizeof(int), cudaMemcpyHostToDevice, st));
+  partition(bl.data(), n_total, n_total, h->n_part_in, in_start, in_order, in_lo, in_hi);
+  BB_CUDA(cudaMemcpyAsync(h->in_idx_dev, in_order.data(), (size_t)n_total * sizeof(int), cudaMemcpyHostToDevice, st));
+  h->pend = 0;
   double gx[kQuad], gw[kQuad];
   gauss_legendre_01(gx, gw);
   const int n_in = h->n_part_in * h->n_part_in, n_out = h->n_part_out * h->n_part_out;
@@ -453,8 +456,8 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
       }
       BB_CUDA(cudaMemsetAsync(h->grid, 0, (size_t)L * n1 * sizeof(float2), st));
       BB_CUDA(cudaMemsetAsync(h->fine, 0, (size_t)L * n2 * sizeof(float2), st));
-      spread_kernel<<<(unsigned)((n_src + 3) / 4), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_dev, n_ant, n_ant,
-                                                                    1.0 / wavelength, h->V, L, g, h->kp, h->grid);
+      spread_kernel<<<(unsigned)((n_src + 3) / 4), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_all_dev, n_ant, h->inv_wl_dev,
+                                                                    h->V, L, g, h->kp, h->grid);
       BB_CUDA(cudaGetLastError());
       deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, decp[0], decp[1], decp[2], h->fine);
       BB_CUDA(cudaGetLastError());
@@ -481,10 +484,58 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
   return BB_OK;
 }
 
+extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
+                                    const float* D, int ldd, const double* xyz, int ldxyz) {
+  if (!h || !B || !D || !xyz || n_ant < 1 || n_ant > 4096 || n_eig < 1 || n_eig > 4096 || !(wavelength > 0.0) || ldb < n_ant ||
+      ldd < h->n_levels || ldxyz < n_ant)
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
+  cudaStream_t st = bb_ctx_user_stream(h->ctx);
+  const int L = h->n_levels;
+  const int64_t n_base = (int64_t)n_ant * n_ant;
+  int rc;
+  if (h->pend > 0 && (h->pend_n_ant != n_ant || (h->pend + 1) * n_base > kMaxPendingSources) && (rc = nufft_flush(h)) != BB_OK) return rc;
+  if ((rc = grow(&h->B_dev, &h->B_cap, (size_t)n_ant * n_eig)) != BB_OK || (rc = grow(&h->D_dev, &h->D_cap, (size_t)L * n_eig)) != BB_OK ||
+      (rc = grow(&h->xyz_dev, &h->xyz_cap, (size_t)3 * n_ant)) != BB_OK)
+    return rc;
+  const size_t v_need = (size_t)(h->pend + 1) * L * n_base;
+  if (v_need > h->V_cap) {                                            // grow and keep the staged collects' visibilities
+    const size_t cap = std::max(v_need, 2 * h->V_cap);
+    float2* nv = nullptr;
+    if (cudaMalloc(&nv, cap * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+    if (h->pend > 0) BB_CUDA(cudaMemcpyAsync(nv, h->V, (size_t)h->pend * L * n_base * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    BB_CUDA(cudaStreamSynchronize(st));
+    cudaFree(h->V);
+    h->V = nv; h->V_cap = cap;
+  }
+  // snapshot the inputs (host or device: unified addressing), compact
+  BB_CUDA(cudaMemcpy2DAsync(h->B_dev, (size_t)n_ant * 8, B, (size_t)ldb * 8, (size_t)n_ant * 8, n_eig, cudaMemcpyDefault, st));
+  BB_CUDA(cudaMemcpy2DAsync(h->D_dev, (size_t)L * 4, D, (size_t)ldd * 4, (size_t)L * 4, n_eig, cudaMemcpyDefault, st));
+  BB_CUDA(cudaMemcpy2DAsync(h->xyz_dev, (size_t)n_ant * 8, xyz, (size_t)ldxyz * 8, (size_t)n_ant * 8, 3, cudaMemcpyDefault, st));
+  vis_kernel<<<(unsigned)((n_base + 255) / 256), 256, 0, st>>>(h->B_dev, n_ant, h->D_dev, L, n_ant, n_eig, L,
+                                                               h->V + (size_t)h->pend * L * n_base);
+  BB_CUDA(cudaGetLastError());
+  std::vector<double> xh((size_t)3 * n_ant);
+  BB_CUDA(cudaMemcpyAsync(xh.data(), h->xyz_dev, xh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BB_CUDA(cudaStreamSynchronize(st));
+  if (h->pend == 0) { h->xyz_all.clear(); h->inv_wl_all.clear(); }
+  const size_t o = h->xyz_all.size();
+  h->xyz_all.resize(o + (size_t)3 * n_ant);
+  for (int p = 0; p < n_ant; ++p) {                                   // antenna positions into the handle's rotated frame
+    const double x = xh[p], y = xh[(size_t)n_ant + p], z = xh[(size_t)2 * n_ant + p];
+    for (int d = 0; d < 3; ++d) h->xyz_all[o + (size_t)d * n_ant + p] = h->R[3 * d] * x + h->R[3 * d + 1] * y + h->R[3 * d + 2] * z;
+  }
+  h->inv_wl_all.push_back(1.0 / wavelength);
+  h->pend += 1; h->pend_n_ant = n_ant;
+  return BB_OK;
+}
+
 extern "C" int bb_nufft_get(bb_nufft* h, int level, float* out) {
   if (!h || !out || level < 0 || level >= h->n_levels) return BB_EINVAL;
   BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
   cudaStream_t st = bb_ctx_user_stream(h->ctx);
+  int rc = nufft_flush(h);
+  if (rc != BB_OK) return rc;
   BB_CUDA(cudaMemcpyAsync(out, h->img + (size_t)level * h->pix_stride, (size_t)h->n_pix * sizeof(float), cudaMemcpyDefault, st));
   BB_CUDA(cudaStreamSynchronize(st));
   return BB_OK;
