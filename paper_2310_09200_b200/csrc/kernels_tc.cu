@@ -394,7 +394,11 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       if (have) {
         if constexpr (C::kLsOnTensor) {
           // ls_full(n) also implies that the MMAs which last read this A stage have completed (same issuer, in order)
-          mbar_wait2(&b_full[sb], pb, &ls_full[2 * sa + tile], pa);
+          // Two waits, not a paired one: the chunk's B stage landed long ago (the ring is kSB deep), so its check costs one
+          // barrier round trip that runs under the wait for ls; the ls loop then polls ONE barrier — the polls of waiting
+          // producer warps were 14 % of all issued instructions with the paired wait (ncu source page, round 2b).
+          mbar_wait(&b_full[sb], pb);
+          mbar_wait(&ls_full[2 * sa + tile], pa);
         } else {
           mbar_wait2(&a_empty[sa], pa ^ 1, &b_full[sb], pb);
         }
