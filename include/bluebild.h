@@ -234,6 +234,12 @@ int bb_nufft_get(bb_nufft* h, int level, float* out);   /* n_pix floats, host or
 /* number of transforms run and the largest fine grid (points) so far: what Section 3.4.1 / Figure 1c is about */
 int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_grid_points);
 
+/* ---- launch-shape query (host only, no device needed) ---------------------------------------------
+ * Number of collect ranges a synthesizer launch over n_collects queued collects is split into on a GPU with sm_count
+ * SMs: 1 = one CTA per pixel tile handles all collects; > 1 for small images whose tile count would leave most of a
+ * wave of SMs empty (the ranges' level sums are added in a fixed order). Returns 0 on invalid arguments. */
+int bb_plan_collect_split(int variant, int64_t n_pix, int n_ant, int n_eig, int n_levels, int n_collects, int sm_count);
+
 const char* bb_status_string(int status);
 const char* bb_version(void);
 

@@ -29,7 +29,7 @@ EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destr
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
            "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version",
-           "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
+           "bb_plan_collect_split", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
 
 _lib = None
 
@@ -76,6 +76,7 @@ def load_library(path: str = LIB_PATH):
         "bb_uvgrid_add": ([vp, i32, f64, vp, i32], i32),
         "bb_uvgrid_destroy": ([vp], i32),
         "bb_synth_set_weighting": ([vp, vp], i32),
+        "bb_plan_collect_split": ([i32, i64, i32, i32, i32, i32, i32], i32),
         "bb_nufft_create": ([vp, i64, vp, i64, i32, f64, i32, i32, pp], i32),
         "bb_nufft_destroy": ([vp], i32),
         "bb_nufft_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
@@ -326,6 +327,12 @@ class StandardSynthesis:
 
     def launches(self) -> int:
         return int(_lib.bb_synth_launches(self._h))
+
+
+def plan_collect_split(variant, n_pix, n_ant, n_eig, n_levels, n_collects, sm_count=148) -> int:
+    """How many collect ranges a launch over n_collects queued collects is split into (host-only query, no device needed)."""
+    load_library()
+    return int(_lib.bb_plan_collect_split(_VARIANTS[variant], int(n_pix), int(n_ant), int(n_eig), int(n_levels), int(n_collects), int(sm_count)))
 
 
 class NufftSynthesis:

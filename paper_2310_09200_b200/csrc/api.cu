@@ -341,6 +341,13 @@ static int launch_queue(bb_synth* s) {
   return BB_OK;
 }
 
+extern "C" int bb_plan_collect_split(int variant, int64_t n_pix, int n_ant, int n_eig, int n_levels, int n_collects, int sm_count) {
+  if (n_pix < 1 || n_ant < 1 || n_eig < 1 || n_levels < 1 || n_collects < 1 || sm_count < 1) return 0;
+  if (variant == BB_VARIANT_FP32) return bb_fp32_split(bb_fp32_plan(n_ant, n_eig, n_levels), n_pix, n_collects, sm_count);
+  if (variant == BB_VARIANT_TF32X3 || variant == BB_VARIANT_FP16X3 || variant == BB_VARIANT_FP16_FP8) return bb_tc_split(n_pix, n_collects, sm_count);
+  return 0;
+}
+
 extern "C" int bb_synth_flush(bb_synth* s) {
   if (!s) return BB_EINVAL;
   BB_CUDA(cudaSetDevice(s->ctx->device));

@@ -1,0 +1,41 @@
+"""Host logic of the collect-range split (csrc/kernels_tc.cu bb_collect_split, through the host-only ABI query
+bb_plan_collect_split; no GPU needed): which launches are split, and that a split always pays in wave efficiency."""
+import numpy as np
+import pytest
+
+from paper_2310_09200_b200 import binding
+
+SM = 148
+# (variant, pixels per CTA, resident CTAs per SM) as the kernels are built: tensor variants 256 / 1; FP32 depends on n_eig
+TENSOR = ("tf32x3", "fp16x3", "fp16fp8")
+
+
+def eff(tiles, split, slots):
+    ctas = tiles * split
+    return ctas / (-(-ctas // slots) * slots)
+
+
+def test_baseline_configs():
+    shapes = {1: (32 * 32, 16, 8, 2, 1), 2: (256 * 256, 1776, 12, 4, 60), 3: (512 * 512, 512, 32, 4, 100),
+              4: (1024 * 1024, 512, 64, 8, 20), 5: (2048 * 2048, 512, 64, 8, 128)}
+    for v in TENSOR:
+        got = {k: binding.plan_collect_split(v, *s) for k, s in shapes.items()}
+        assert got == {1: 1, 2: 4, 3: 1, 4: 1, 5: 1}, (v, got)      # config 2: 256 tiles x 4 = 6.92 waves of 148 SMs
+    got = {k: binding.plan_collect_split("fp32", *s) for k, s in shapes.items()}
+    assert got[1] == 1 and got[2] == 2 and got[4] == 1 and got[5] == 1, got
+
+
+def test_split_rules():
+    rng = np.random.default_rng(5)
+    for _ in range(400):
+        n_pix = int(rng.integers(1, 600_000)); n_col = int(rng.integers(1, 129)); sm = int(rng.choice([148, 132, 80, 16]))
+        s = binding.plan_collect_split("fp16fp8", n_pix, 64, 16, 2, n_col, sm)
+        tiles = -(-n_pix // 256)
+        assert 1 <= s <= 8
+        if s > 1:
+            assert n_col // s >= 4                                   # every range keeps at least 4 collects
+            assert eff(tiles, s, sm) > eff(tiles, 1, sm) + 0.05      # a split must pay
+            assert eff(tiles, 1, sm) < 0.95
+        if n_col < 8 or eff(tiles, 1, sm) >= 0.95:
+            assert s == 1
+    assert binding.plan_collect_split("fp16fp8", 0, 64, 16, 2, 10, 148) == 0      # invalid arguments
