@@ -337,7 +337,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
     const int l = i / NE, k = i - l * NE;
     dsm[i] = weights[(size_t)l * n_eig_pad + eig_offset + k];
   }
-  // per-pixel constants of the phase generator (producer threads; both groups own the same 256 pixels)
+  // per-pixel constants of the phase generator (producer threads; all groups own the same 256 pixels)
   const int slot = tid & (kTilePixels - 1);                // pixel of the CTA: tile * 128 + quadrant * 32 + lane
   const int64_t j = (int64_t)blockIdx.x * kTilePixels + slot;
   const bool ok = warp < kProducerWarps && j < n_pix;
@@ -357,7 +357,7 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
   if (warp < kProducerWarps) {
     // ===================== producers / epilogue: one pixel (TMEM lane) per thread =====================
     const int group = warp >> 3, tile = (warp >> 2) & 1;
-    const int ptid = tid;                                  // 0..511 over both groups
+    const int ptid = tid;                                  // 0 .. 256 G - 1 over all groups
     const uint32_t lane_field = (uint32_t)((warp & 3) * 32) << 16;
     if (C::kLsOnTensor && group == 0) {
       // A operand of the mini-GEMM in TMEM, row = pixel, K = 16 halves in 8 columns:
@@ -540,8 +540,8 @@ synth_tc_kernel(const double* __restrict__ rprime, int64_t n_pix, int64_t pix_st
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0;                             // phase parities of the A / B stage rings
       // mini-GEMM (FP16 mode): ls[pixel, antenna] = sum_d (2 pi PH_d RL_d + 2 pi PL_d r'_d) - 2 pi for the 16
-      // antennas of chunk m, written into the lo half of A stage m % kSA two chunks ahead of the main MMAs of
-      // chunk m. The stage was last read by the main MMAs of chunk m - kSA, issued earlier by this same thread:
+      // antennas of chunk m, written into the lo half of A stage m % kSA, kSA chunks ahead of the main MMAs of
+      // chunk m. The stage was last read by the main MMAs of chunk m - kSA, issued just before by this same thread:
       // the tensor pipe executes one thread's MMAs in order, so no barrier is needed to reuse the columns, and
       // ls_full(m) tells the producers both "ls is there" and "the stage is free".
       const uint32_t idesc_ls = (1u << 4) | ((uint32_t)(kAC >> 3) << 17) | ((128u >> 4) << 24);
