@@ -220,7 +220,7 @@ int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int
  * eps: requested relative tolerance (1e-2 .. 1e-7; sets the kernel width). pix as for bb_synth_create (host or
  * device). B, D, xyz: host or device, as bb_synth_collect_eig; the call snapshots them, forms V'_l on the device and
  * STAGES the collect (it synchronises the context stream). The transforms run in bb_nufft_get — ONE set over the
- * baselines of all staged collects, the paper's use of the NUFFT over all time steps — or earlier when 2^25 staged
+ * baselines of all staged collects, the paper's use of the NUFFT over all time steps — or earlier when 2^24 staged
  * baselines are reached or n_ant changes. BB_EUNSUPPORTED (from the call that runs the transforms; the staged
  * collects are dropped): a pair's fine grid would exceed 2^28 points: raise the partition counts.
  * Same images as bb_synth_collect_eig up to eps; O(n_ant^2 L w^3 + grid log grid + n_pix L w^3) per pair. */

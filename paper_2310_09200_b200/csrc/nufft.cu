@@ -381,7 +381,7 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
   return BB_OK;
 }
 
-constexpr int64_t kMaxPendingSources = (int64_t)1 << 25;
+constexpr int64_t kMaxPendingSources = (int64_t)1 << 24;   // host bookkeeping: 24 B of coordinates + 4 B of index per staged baseline
 
 // One set of transforms over the baselines of all staged collects (Eq. 36 over cells; the sum over time steps is just more sources).
 static int nufft_flush(bb_nufft* h) {

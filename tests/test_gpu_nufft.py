@@ -109,3 +109,20 @@ def test_argument_validation_and_grid_limit(bb, ctx):
     with pytest.raises(bb.BluebildError) as e:
         h.images()                                                          # the transforms run here
     assert e.value.code == 7                                                # BB_EUNSUPPORTED: raise the partition counts
+
+
+def test_staging_flushes_when_the_array_changes(bb, ctx, oracle):
+    """Staged collects share one source list only while n_ant stays the same: a different array runs the pending transforms first."""
+    ca = case(41, 12, 5, 2, 24, 300.0, np.deg2rad(8.0))
+    cb = case(42, 20, 7, 2, 24, 500.0, np.deg2rad(8.0))
+    pix = ca["pix"]
+    ref = oracle.nufft_direct(ca["B"], ca["D"], ca["xyz"], pix, ca["wavelength"])[0]
+    ref = ref + oracle.nufft_direct(cb["B"], cb["D"], cb["xyz"], pix, cb["wavelength"])[0]
+    ref = ref + oracle.nufft_direct(ca["B"], ca["D"], ca["xyz"], pix, ca["wavelength"])[0]
+    h = bb.NufftSynthesis(ctx, pix, 2, eps=1e-6, n_part_in=2, n_part_out=2)
+    h.collect_eig(ca["B"], ca["D"], ca["xyz"], ca["wavelength"])
+    assert h.stats()["n_transforms"] == 0
+    h.collect_eig(cb["B"], cb["D"], cb["xyz"], cb["wavelength"])          # 20 antennas: the 12-antenna collect is transformed now
+    assert h.stats()["n_transforms"] > 0
+    h.collect_eig(ca["B"], ca["D"], ca["xyz"], ca["wavelength"])
+    assert_parity(h.images(), ref, "NUFFT synthesis, arrays of 12 / 20 / 12 antennas")
