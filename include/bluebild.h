@@ -222,7 +222,7 @@ int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int
  * STAGES the collect (it synchronises the context stream). The transforms run in bb_nufft_get — ONE set over the
  * baselines of all staged collects, the paper's use of the NUFFT over all time steps — or earlier when 2^24 staged
  * baselines are reached or n_ant changes. BB_EUNSUPPORTED (from the call that runs the transforms; the staged
- * collects are dropped): a pair's fine grid would exceed 2^28 points: raise the partition counts.
+ * collects are dropped): a pair's fine grids (all levels, complex64) would exceed 32 GB: raise the partition counts.
  * Same images as bb_synth_collect_eig up to eps; O(n_ant^2 L w^3 + grid log grid + n_pix L w^3) per pair. */
 typedef struct bb_nufft bb_nufft;
 int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pix, int n_levels, double eps,
@@ -233,6 +233,13 @@ int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, c
 int bb_nufft_get(bb_nufft* h, int level, float* out);   /* n_pix floats, host or device; synchronises */
 /* number of transforms run and the largest fine grid (points) so far: what Section 3.4.1 / Figure 1c is about */
 int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_grid_points);
+
+/* Host-only planning query (no device needed; pix and xyz must be HOST pointers): the transforms ONE collect of this
+ * array would need under an (n_part_in, n_part_out) partitioning — their number, the largest and the summed fine-grid
+ * sizes (points, per level) and the fraction of non-empty input cells: the quantities of Section 3.4.1 / Figure 1c-d. */
+int bb_nufft_plan(int64_t n_pix, const double* pix, int64_t ld_pix, int n_ant, const double* xyz, int ldxyz, double wavelength,
+                  double eps, int n_part_in, int n_part_out, int64_t* n_transforms, int64_t* max_grid_points,
+                  double* sum_grid_points, double* nonempty_input_cells);
 
 /* ---- launch-shape query (host only, no device needed) ---------------------------------------------
  * Number of collect ranges a synthesizer launch over n_collects queued collects is split into on a GPU with sm_count

@@ -29,7 +29,7 @@ EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destr
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
            "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version",
-           "bb_plan_collect_split", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
+           "bb_plan_collect_split", "bb_nufft_plan", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
 
 _lib = None
 
@@ -77,6 +77,7 @@ def load_library(path: str = LIB_PATH):
         "bb_uvgrid_destroy": ([vp], i32),
         "bb_synth_set_weighting": ([vp, vp], i32),
         "bb_plan_collect_split": ([i32, i64, i32, i32, i32, i32, i32], i32),
+        "bb_nufft_plan": ([i64, vp, i64, i32, vp, i32, f64, f64, i32, i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64), pd, pd], i32),
         "bb_nufft_create": ([vp, i64, vp, i64, i32, f64, i32, i32, pp], i32),
         "bb_nufft_destroy": ([vp], i32),
         "bb_nufft_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
@@ -333,6 +334,16 @@ def plan_collect_split(variant, n_pix, n_ant, n_eig, n_levels, n_collects, sm_co
     """How many collect ranges a launch over n_collects queued collects is split into (host-only query, no device needed)."""
     load_library()
     return int(_lib.bb_plan_collect_split(_VARIANTS[variant], int(n_pix), int(n_ant), int(n_eig), int(n_levels), int(n_collects), int(sm_count)))
+
+
+def nufft_plan(pix, xyz, wavelength, eps=1e-6, n_part_in=1, n_part_out=1):
+    """Host-only (Section 3.4.1): transforms, largest / summed fine-grid points and non-empty input-cell fraction of one collect."""
+    load_library()
+    P = np.asfortranarray(np.asarray(pix, dtype=np.float64)); X = np.asfortranarray(np.asarray(xyz, dtype=np.float64))
+    nt, mx, sm, ne = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_double(), ctypes.c_double()
+    _check(_lib.bb_nufft_plan(P.shape[0], P.ctypes.data, P.shape[0], X.shape[0], X.ctypes.data, X.shape[0], float(wavelength), float(eps),
+                              int(n_part_in), int(n_part_out), ctypes.byref(nt), ctypes.byref(mx), ctypes.byref(sm), ctypes.byref(ne)), "bb_nufft_plan")
+    return dict(n_transforms=nt.value, max_grid_points=mx.value, sum_grid_points=sm.value, nonempty_input_cells=ne.value)
 
 
 class NufftSynthesis:

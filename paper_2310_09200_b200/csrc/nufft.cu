@@ -30,7 +30,7 @@ namespace {
 constexpr int kMaxW = 12;               // kernel width (grid points) at most
 constexpr int kQuad = 32;               // Gauss-Legendre nodes on [0, 1] for the kernel's Fourier transform
 constexpr double kSigma = 2.0;          // upsampling of both stages
-constexpr int64_t kMaxGrid = (int64_t)1 << 28;
+constexpr double kMaxGridBytes = 32e9;     // fine grids of all levels of one transform (complex64)
 
 __constant__ double c_gl_x[kQuad], c_gl_w[kQuad];
 
@@ -303,6 +303,51 @@ void partition(const double* c, int64_t n, int64_t ld, int parts, std::vector<in
   }
 }
 
+// Frame (e_u, e_v, e_w) with e_w = the mean pixel direction (rows of R); the pixels ([3][n]) are rotated in place.
+void rotate_to_mean_direction(std::vector<double>& pix, int64_t n_pix, double R[9]) {
+  double m[3] = {0, 0, 0};
+  for (int d = 0; d < 3; ++d) { for (int64_t i = 0; i < n_pix; ++i) m[d] += pix[(size_t)d * n_pix + i]; }
+  const double nm = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+  if (nm > 1e-12 * (double)n_pix) {
+    for (int d = 0; d < 3; ++d) R[6 + d] = m[d] / nm;
+    int k = 0;                                                      // the coordinate axis least aligned with e_w
+    for (int d = 1; d < 3; ++d) if (fabs(R[6 + d]) < fabs(R[6 + k])) k = d;
+    double a[3] = {0, 0, 0};
+    a[k] = 1.0;
+    const double dot = R[6 + k];
+    double u[3], un = 0;
+    for (int d = 0; d < 3; ++d) { u[d] = a[d] - dot * R[6 + d]; un += u[d] * u[d]; }
+    un = sqrt(un);
+    for (int d = 0; d < 3; ++d) R[d] = u[d] / un;
+    R[3] = R[7] * R[2] - R[8] * R[1]; R[4] = R[8] * R[0] - R[6] * R[2]; R[5] = R[6] * R[1] - R[7] * R[0];   // e_v = e_w x e_u
+  }
+  for (int64_t i = 0; i < n_pix; ++i) {
+    const double x = pix[i], y = pix[(size_t)n_pix + i], z = pix[(size_t)2 * n_pix + i];
+    for (int d = 0; d < 3; ++d) pix[(size_t)d * n_pix + i] = R[3 * d] * x + R[3 * d + 1] * y + R[3 * d + 2] * z;
+  }
+}
+
+// Grids of one (input cell, output cell) pair from the cells' bounding boxes (x in wavelengths, r as pixel coordinates).
+void pair_geometry(const double* xlo, const double* xhi, const double* rlo, const double* rhi, int w, CellGeom& g, int64_t& n1, int64_t& n2) {
+  n1 = 1; n2 = 1;
+  for (int d = 0; d < 3; ++d) {
+    const double xl = xlo[d], xu = xhi[d];
+    const double sl = -6.283185307179586 * rhi[d], su = -6.283185307179586 * rlo[d];
+    g.xc[d] = 0.5 * (xl + xu); g.sc[d] = 0.5 * (sl + su);
+    const double X = std::max(0.5 * (xu - xl), 1e-9), S = std::max(0.5 * (su - sl), 1e-9);
+    // at least one grid point per unit of X S beyond the minimum, so that degenerate (thin) dimensions stay tiny
+    const double XS = std::max(X * S, 0.5);
+    const double S_eff = XS / X;                                    // S widened when X S is tiny: theta stays within +-pi/sigma
+    g.nf1[d] = next_smooth_even(std::max(2 * w, (int)ceil(2.0 * kSigma * X * S_eff / 3.141592653589793) + w + 2));
+    g.nf2[d] = next_smooth_even(std::max(2 * w, (int)ceil(kSigma * g.nf1[d])));
+    g.pos_scale[d] = kSigma * S_eff / 3.141592653589793;
+    g.theta_scale[d] = 3.141592653589793 / (kSigma * S_eff);
+    n1 *= g.nf1[d]; n2 *= g.nf2[d];
+  }
+}
+
+int kernel_width(double eps) { return std::min(kMaxW, std::max(2, (int)ceil(-log10(eps / 10.0)) + 1)); }
+
 }  // namespace
 
 extern "C" int bb_nufft_destroy(bb_nufft* h) {
@@ -332,7 +377,7 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
   bb_ctx_ref(ctx, +1);
   h->n_part_in = n_part_in; h->n_part_out = n_part_out;
   // kernel width from the tolerance (one more grid point per decade, as FINUFFT's rule for sigma = 2), beta = 2.30 w
-  h->kp.w = std::min(kMaxW, std::max(2, (int)ceil(-log10(eps / 10.0)) + 1));
+  h->kp.w = kernel_width(eps);
   h->kp.beta = 2.30 * h->kp.w;
   double gx[kQuad], gw[kQuad];
   gauss_legendre_01(gx, gw);
@@ -347,29 +392,7 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
     if (cudaMalloc(&h->pix_dev, (size_t)3 * n_pix * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&h->img, (size_t)n_levels * h->pix_stride * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&h->out_idx_dev, (size_t)n_pix * sizeof(int)) != cudaSuccess) { rc = BB_EALLOC; break; }
-    {   // rotate the pixels into (e_u, e_v, e_w)
-      double m[3] = {0, 0, 0};
-      for (int d = 0; d < 3; ++d) { for (int64_t i = 0; i < n_pix; ++i) m[d] += h->pix_host[(size_t)d * n_pix + i]; }
-      double nm = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
-      if (nm > 1e-12 * (double)n_pix) {
-        double* R = h->R;
-        for (int d = 0; d < 3; ++d) R[6 + d] = m[d] / nm;
-        int k = 0;                                                    // the coordinate axis least aligned with e_w
-        for (int d = 1; d < 3; ++d) if (fabs(R[6 + d]) < fabs(R[6 + k])) k = d;
-        double a[3] = {0, 0, 0};
-        a[k] = 1.0;
-        const double dot = R[6 + k];
-        double u[3], un = 0;
-        for (int d = 0; d < 3; ++d) { u[d] = a[d] - dot * R[6 + d]; un += u[d] * u[d]; }
-        un = sqrt(un);
-        for (int d = 0; d < 3; ++d) R[d] = u[d] / un;
-        R[3] = R[7] * R[2] - R[8] * R[1]; R[4] = R[8] * R[0] - R[6] * R[2]; R[5] = R[6] * R[1] - R[7] * R[0];   // e_v = e_w x e_u
-      }
-      for (int64_t i = 0; i < n_pix; ++i) {
-        const double x = h->pix_host[i], y = h->pix_host[(size_t)n_pix + i], z = h->pix_host[(size_t)2 * n_pix + i];
-        for (int d = 0; d < 3; ++d) h->pix_host[(size_t)d * n_pix + i] = h->R[3 * d] * x + h->R[3 * d + 1] * y + h->R[3 * d + 2] * z;
-      }
-    }
+    rotate_to_mean_direction(h->pix_host, n_pix, h->R);
     std::vector<int> order;
     partition(h->pix_host.data(), n_pix, n_pix, n_part_out, h->out_start, order, h->out_lo, h->out_hi);
     if (cudaMemcpy(h->pix_dev, h->pix_host.data(), (size_t)3 * n_pix * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -421,22 +444,9 @@ static int nufft_flush(bb_nufft* h) {
       const int n_tgt = h->out_start[oc + 1] - h->out_start[oc];
       if (n_tgt == 0) continue;
       CellGeom g{};
-      int64_t n1 = 1, n2 = 1;
-      for (int d = 0; d < 3; ++d) {
-        const double xl = in_lo[ic * 3 + d], xu = in_hi[ic * 3 + d];
-        const double sl = -6.283185307179586 * h->out_hi[oc * 3 + d], su = -6.283185307179586 * h->out_lo[oc * 3 + d];
-        g.xc[d] = 0.5 * (xl + xu); g.sc[d] = 0.5 * (sl + su);
-        const double X = std::max(0.5 * (xu - xl), 1e-9), S = std::max(0.5 * (su - sl), 1e-9);
-        // at least one grid point per unit of X S beyond the minimum, so that degenerate (thin) dimensions stay tiny
-        const double XS = std::max(X * S, 0.5);
-        const double S_eff = XS / X;                                  // S widened when X S is tiny: theta stays within +-pi/sigma
-        g.nf1[d] = next_smooth_even(std::max(2 * w, (int)ceil(2.0 * kSigma * X * S_eff / 3.141592653589793) + w + 2));
-        g.nf2[d] = next_smooth_even(std::max(2 * w, (int)ceil(kSigma * g.nf1[d])));
-        g.pos_scale[d] = kSigma * S_eff / 3.141592653589793;
-        g.theta_scale[d] = 3.141592653589793 / (kSigma * S_eff);
-        n1 *= g.nf1[d]; n2 *= g.nf2[d];
-      }
-      if (n2 > kMaxGrid) return BB_EUNSUPPORTED;
+      int64_t n1, n2;
+      pair_geometry(&in_lo[ic * 3], &in_hi[ic * 3], &h->out_lo[oc * 3], &h->out_hi[oc * 3], w, g, n1, n2);
+      if ((double)n2 * L * 8.0 > kMaxGridBytes || n2 > 0x7fffffffLL) return BB_EUNSUPPORTED;
       if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * n2)) != BB_OK)
         return rc;                                                    // (cudaFree of a buffer in use waits for the device)
       // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step): one device array per (nf1, nf2), kept
@@ -545,5 +555,49 @@ extern "C" int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_g
   if (!h) return BB_EINVAL;
   if (n_transforms) *n_transforms = h->n_transforms;
   if (max_grid_points) *max_grid_points = h->max_grid;
+  return BB_OK;
+}
+
+
+// Host-only: what Section 3.4.1 / Figure 1c-d is about — the transforms one collect would need, without running them.
+extern "C" int bb_nufft_plan(int64_t n_pix, const double* pix, int64_t ld_pix, int n_ant, const double* xyz, int ldxyz, double wavelength,
+                             double eps, int n_part_in, int n_part_out, int64_t* n_transforms, int64_t* max_grid_points,
+                             double* sum_grid_points, double* nonempty_input_cells) {
+  if (n_pix < 1 || n_pix > 0x7fffffff || !pix || ld_pix < n_pix || n_ant < 1 || n_ant > 4096 || !xyz || ldxyz < n_ant || !(wavelength > 0.0) ||
+      !(eps >= 1e-7 && eps <= 1e-2) || n_part_in < 1 || n_part_in > 64 || n_part_out < 1 || n_part_out > 64)
+    return BB_EINVAL;
+  std::vector<double> ph((size_t)3 * n_pix);
+  for (int d = 0; d < 3; ++d) for (int64_t i = 0; i < n_pix; ++i) ph[(size_t)d * n_pix + i] = pix[(size_t)d * ld_pix + i];
+  double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+  rotate_to_mean_direction(ph, n_pix, R);
+  std::vector<int> out_start, order, in_start, in_order;
+  std::vector<double> out_lo, out_hi, in_lo, in_hi;
+  partition(ph.data(), n_pix, n_pix, n_part_out, out_start, order, out_lo, out_hi);
+  const int64_t n_base = (int64_t)n_ant * n_ant;
+  std::vector<double> xr((size_t)3 * n_ant), bl((size_t)3 * n_base);
+  for (int p = 0; p < n_ant; ++p)
+    for (int d = 0; d < 3; ++d) xr[(size_t)d * n_ant + p] = R[3 * d] * xyz[p] + R[3 * d + 1] * xyz[(size_t)ldxyz + p] + R[3 * d + 2] * xyz[(size_t)2 * ldxyz + p];
+  for (int d = 0; d < 3; ++d)
+    for (int q = 0; q < n_ant; ++q)
+      for (int p = 0; p < n_ant; ++p) bl[(size_t)d * n_base + p + (size_t)n_ant * q] = (xr[(size_t)d * n_ant + p] - xr[(size_t)d * n_ant + q]) / wavelength;
+  partition(bl.data(), n_base, n_base, n_part_in, in_start, in_order, in_lo, in_hi);
+  const int w = kernel_width(eps), n_in = n_part_in * n_part_in, n_out = n_part_out * n_part_out;
+  int64_t nt = 0, mx = 0, occupied = 0;
+  double sum = 0.0;
+  for (int ic = 0; ic < n_in; ++ic) {
+    if (in_start[ic + 1] == in_start[ic]) continue;
+    ++occupied;
+    for (int oc = 0; oc < n_out; ++oc) {
+      if (out_start[oc + 1] == out_start[oc]) continue;
+      CellGeom g{};
+      int64_t n1, n2;
+      pair_geometry(&in_lo[ic * 3], &in_hi[ic * 3], &out_lo[oc * 3], &out_hi[oc * 3], w, g, n1, n2);
+      ++nt; mx = std::max(mx, n2); sum += (double)n2;
+    }
+  }
+  if (n_transforms) *n_transforms = nt;
+  if (max_grid_points) *max_grid_points = mx;
+  if (sum_grid_points) *sum_grid_points = sum;
+  if (nonempty_input_cells) *nonempty_input_cells = (double)occupied / n_in;
   return BB_OK;
 }

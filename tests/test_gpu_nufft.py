@@ -126,3 +126,27 @@ def test_staging_flushes_when_the_array_changes(bb, ctx, oracle):
     assert h.stats()["n_transforms"] > 0
     h.collect_eig(ca["B"], ca["D"], ca["xyz"], ca["wavelength"])
     assert_parity(h.images(), ref, "NUFFT synthesis, arrays of 12 / 20 / 12 antennas")
+
+
+def test_config3_two_collects_partitioned(bb, ctx, oracle):
+    """BASELINE config 3 (512 stations to 35 km, 512 x 512 pixels over 15 degrees): unpartitioned, one transform would need a
+    2.3e12-point fine grid per level (18 TB); 64 x 64 input cells bring the largest grid to 2e7 points (Section 3.4.1). Two collects
+    are staged and transformed together; the whole image is synthesized, the every-16th subset + brightest-source pixels
+    are compared with the oracle's Standard Synthesis (= Eq. 19, pinned)."""
+    from paper_2310_09200_b200 import workloads
+    from helpers import eig_inputs, intervals_for
+    w = workloads.make_workload(3)
+    iv = intervals_for(oracle, workloads, w, [0, 50])
+    items = [eig_inputs(oracle, workloads, w, n, iv) for n in (0, 50)]        # 3 hours apart: the union of two baseline clouds
+    plan1 = bb.nufft_plan(w.pixels(), items[0]["xyz"], items[0]["wavelength"], 1e-5, 1, 1)
+    plan64 = bb.nufft_plan(w.pixels(), items[0]["xyz"], items[0]["wavelength"], 1e-5, 64, 1)
+    assert plan1["max_grid_points"] > 1e12 and plan64["max_grid_points"] < 1e8 and plan64["nonempty_input_cells"] < 0.7
+    sub = w.sample_pixels(16)
+    ref = np.zeros((w.cfg.n_levels, sub.size))
+    for it in items:
+        oracle.synth(it["B"], it["D"], it["xyz"], w.pixels(sub), it["wavelength"], img=ref)
+    h = bb.NufftSynthesis(ctx, w.pixels(), w.cfg.n_levels, eps=1e-5, n_part_in=64, n_part_out=1)
+    for it in items:
+        h.collect_eig(it["B"], it["D"], it["xyz"], it["wavelength"])
+    got = h.images()
+    assert_parity(got[:, sub], ref, "NUFFT synthesis config 3")
