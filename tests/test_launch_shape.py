@@ -39,3 +39,29 @@ def test_split_rules():
         if n_col < 8 or eff(tiles, 1, sm) >= 0.95:
             assert s == 1
     assert binding.plan_collect_split("fp16fp8", 0, 64, 16, 2, 10, 148) == 0      # invalid arguments
+
+
+def test_nufft_plan_domain_partitioning():
+    """bb_nufft_plan (host only): Section 3.4.1 — partitioning the baselines shrinks the FFT grids by orders of magnitude and
+    leaves a growing share of the partition cells empty (Figure 1c-d), on the synthetic SKA-Low layout of config 3."""
+    from paper_2310_09200_b200 import workloads
+    w1 = workloads.make_workload(1)
+    p = binding.nufft_plan(w1.pixels(), w1.xyz(0), 2.0, 1e-6, 1, 1)
+    assert p["n_transforms"] == 1 and p["max_grid_points"] < 1e6 and p["nonempty_input_cells"] == 1.0
+    w3 = workloads.make_workload(3)
+    pix, xyz = w3.pixels(), w3.xyz(0)
+    prev = None
+    for parts in (1, 4, 16, 64):
+        p = binding.nufft_plan(pix, xyz, 3.0, 1e-4, parts, 1)
+        assert p["n_transforms"] <= parts * parts
+        if prev is not None:
+            assert p["max_grid_points"] < prev["max_grid_points"] / 8 and p["nonempty_input_cells"] <= prev["nonempty_input_cells"]
+        prev = p
+    assert binding.nufft_plan(pix, xyz, 3.0, 1e-4, 1, 1)["max_grid_points"] > 1e12          # 18 TB per level: does not fit anywhere
+    assert prev["max_grid_points"] < 5e7 and 0.3 < prev["nonempty_input_cells"] < 0.7
+    # output partitioning multiplies the transforms and shrinks the grids further
+    q = binding.nufft_plan(pix, xyz, 3.0, 1e-4, 16, 4)
+    assert q["n_transforms"] == 16 * binding.nufft_plan(pix, xyz, 3.0, 1e-4, 16, 1)["n_transforms"]
+    assert q["max_grid_points"] < binding.nufft_plan(pix, xyz, 3.0, 1e-4, 16, 1)["max_grid_points"] / 4
+    with pytest.raises(binding.BluebildError):
+        binding.nufft_plan(pix, xyz, 3.0, 1e-9, 1, 1)
