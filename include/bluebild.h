@@ -209,6 +209,32 @@ int bb_estimate_n_eig(bb_ctx* ctx, const double* lambda, int n, double energy_fr
 int bb_kmeans_levels(bb_ctx* ctx, const double* lambda, int n, int n_levels, int log_domain,
                      double* intervals_out, int ld_int);
 
+/* bb_kmeans_levels_static: bb_kmeans_levels (same kernel, same result) for callers that cannot
+ * allocate device memory when they make the call: a service that laid out all of its GPU memory at start-up (a
+ * streaming imager with a fixed memory plan; a process whose framework pool already owns nearly all of HBM, where
+ * a raw cudaMalloc may simply fail), or a latency-bound loop, since cudaMalloc / cudaFree lock the whole device and
+ * wait for it to go idle, stalling unrelated streams. It calls no cudaMalloc, cudaFree or allocating library
+ * routine and needs no bb_ctx. Its dynamic-programming tables sit in a fixed array inside the library image instead:
+ * about 170 KB that every GPU which loads the library holds until the process exits — hence the lower size limit.
+ *   device, cuda_stream  CUDA ordinal (made current, as bb_ctx_create does; 0..63) and the cudaStream_t (NULL =
+ *                        default stream) the kernel is enqueued on. The call does not synchronise.
+ *   lambda_dev           n eigenvalues, any order, DEVICE memory, 1 <= n <= BB_KMEANS_STATIC_MAX_N.
+ *   intervals_dev        out, DEVICE memory, n_levels x 2 column-major with ld_int >= n_levels, as bb_kmeans_levels.
+ *   status_dev           out, DEVICE int: 0 = intervals written; 1 = fewer than n_levels positive eigenvalues,
+ *                        intervals untouched (the case bb_kmeans_levels reports as BB_EINVAL). Read it in stream order.
+ * All three buffers are the caller's, read and written in stream order on cuda_stream; host pointers are refused
+ * with BB_EINVAL (staging them would take memory). n > BB_KMEANS_STATIC_MAX_N: BB_EUNSUPPORTED, nothing launched
+ * (BB_VERBOSE=1 prints the limit) — use bb_kmeans_levels. Other bad arguments: BB_EINVAL.
+ * First call per device = set-up: it looks up the device address of the built-in array (and may bring up the
+ * device's primary context and load the module). Make that call once, early, before any stream capture begins.
+ * Sharing: every call on a GPU uses the same array. Nothing in it needs clearing (the kernel writes each table
+ * entry before reading it; what the previous call left is never read), but calls whose kernels OVERLAP on one GPU
+ * — different streams, or threads using different streams — race on it. Keep them on one stream, or order them
+ * with events. */
+#define BB_KMEANS_STATIC_MAX_N 1024
+int bb_kmeans_levels_static(int device, void* cuda_stream, const double* lambda_dev, int n, int n_levels,
+                            int log_domain, double* intervals_dev, int ld_int, int* status_dev);
+
 /* ---- NUFFT Synthesis (Section 2.5 Eq. 17-21, Section 3.4 Eq. 32-36, Algorithm 3), SURVEY 8(f) row 3 -----
  * Per collect: V'_l = B diag(D[l,:]) B^H (Eq. 17 with the level selection of Eq. 21; Alg. 3 l.8) on the n_ant^2
  * baselines b_pq = (x_p - x_q) / wavelength, then I_l(r_j) += sum_pq V'_l,pq exp(-2 pi i <b_pq, r_j>) (Eq. 18-19,

@@ -28,7 +28,7 @@ _VARIANTS = {"fp32": VARIANT_FP32, "tf32x3": VARIANT_TF32X3, "fp16x3": VARIANT_F
 EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destroy", "bb_synth_reset",
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
-           "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_status_string", "bb_version",
+           "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_kmeans_levels_static", "bb_status_string", "bb_version",
            "bb_plan_collect_split", "bb_nufft_plan", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
 
 _lib = None
@@ -70,6 +70,7 @@ def load_library(path: str = LIB_PATH):
         "bb_eig": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, vp, i32], i32),
         "bb_estimate_n_eig": ([vp, vp, i32, f64, ctypes.POINTER(ctypes.c_int)], i32),
         "bb_kmeans_levels": ([vp, vp, i32, i32, i32, vp, i32], i32),
+        "bb_kmeans_levels_static": ([i32, vp, vp, i32, i32, i32, vp, i32, vp], i32),
         "bb_synth_status": ([vp], i32),
         "bb_level_weights": ([vp, vp, i32, vp, i32, i32, i32, vp, vp, i32], i32),
         "bb_uvgrid_create": ([vp, f64, vp, vp, f64, pp], i32),
@@ -328,6 +329,27 @@ class StandardSynthesis:
 
     def launches(self) -> int:
         return int(_lib.bb_synth_launches(self._h))
+
+
+KMEANS_STATIC_MAX_N = 1024   # BB_KMEANS_STATIC_MAX_N
+
+
+def kmeans_levels_static(device: int, stream: int, lambda_ptr: int, n: int, n_levels: int, log_domain: bool,
+                         intervals_ptr: int, ld_int: int, status_ptr: int) -> None:
+    """bb_kmeans_levels_static: PAPER.md:164 level intervals for callers that must not allocate GPU memory at call
+    time (fixed memory plan, a framework pool that owns HBM, latency-bound loops that cannot afford cudaMalloc's
+    device-wide stall). Everything is the caller's and on the device: `lambda_ptr` n float64 values, `intervals_ptr`
+    n_levels x 2 float64 column-major with leading dimension ld_int, `status_ptr` one int32 (0 = written, 1 = fewer
+    positive eigenvalues than levels); `stream` is a cudaStream_t as an integer (0 = default stream). Enqueues and
+    returns without synchronising and without allocating here either: pass raw addresses (tensor.data_ptr()).
+    n above KMEANS_STATIC_MAX_N raises BluebildError code 7. The first call on a device does a one-time address
+    look-up: make it before any stream capture. Calls that overlap on one GPU share the scratch and race."""
+    load_library()
+    code = _lib.bb_kmeans_levels_static(int(device), stream or None, lambda_ptr, int(n), int(n_levels), int(bool(log_domain)),
+                                        intervals_ptr, int(ld_int), status_ptr)
+    if code == 7:
+        raise BluebildError(code, "bb_kmeans_levels_static (n = %d, limit %d eigenvalues)" % (n, KMEANS_STATIC_MAX_N))
+    _check(code, "bb_kmeans_levels_static")
 
 
 def plan_collect_split(variant, n_pix, n_ant, n_eig, n_levels, n_collects, sm_count=148) -> int:

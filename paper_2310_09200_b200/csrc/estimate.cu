@@ -11,6 +11,9 @@
 #include "internal.h"
 
 #include <cfloat>
+#include <cstdio>
+#include <cstdlib>
+#include <mutex>
 
 namespace {
 
@@ -156,4 +159,77 @@ int bb_kmeans_levels_dev(const double* lam_dev, int n, int k, int log_domain, do
   kmeans_kernel<<<1, kEstThreads, (size_t)m * sizeof(double), st>>>(lam_dev, n, m, k, log_domain, ws, arg, iv_dev, ld_int, status_dev);
   BB_CUDA(cudaGetLastError());
   return BB_OK;
+}
+
+// ------------------------------------------------------------------------------ k-means levels without allocation
+// bb_kmeans_levels_static: the same kmeans_kernel, for callers that must not allocate device memory at call time.
+// Who that is: an imaging service that sized all of its device memory when it started (a streaming telescope back end
+// with a fixed memory plan, or a process in which a framework's caching pool already holds nearly all of HBM, so a
+// raw cudaMalloc can simply fail), and any latency-bound loop, because cudaMalloc / cudaFree take a device-wide lock
+// and make the whole GPU idle before they return, stalling streams that have nothing to do with this call.
+// bb_kmeans_levels above allocates four scratch buffers per call; here the dynamic-programming tables live in ONE
+// array that is part of the loaded library image. Cost: every GPU that loads the library carries these
+// kStaticBytes (about 170 KB) until the process exits, and the problem size is capped at BB_KMEANS_STATIC_MAX_N.
+//
+// The array's name below is only a host-side handle of the symbol: handed to a kernel from host code it is NOT the
+// device address. The address is asked for once per device (cudaGetSymbolAddress, with that device current) and
+// cached; this happens in the first call made for a device, which is therefore the set-up call (make it once,
+// early, before any stream capture; it may initialise the device's primary context and load the module).
+//
+// All calls on one GPU share the array. kmeans_kernel writes every table entry before it reads it (x, p1, p2 and
+// the dp / arg rows up to the np of THIS call), so nothing has to be cleared between calls and the contents a
+// previous call left behind are never read. Two calls whose kernels overlap on the same GPU (different streams,
+// or different host threads on different streams) race on the tables: serialise them on one stream.
+namespace {
+
+constexpr int kStaticM = BB_KMEANS_STATIC_MAX_N;                                    // a power of two
+static_assert((kStaticM & (kStaticM - 1)) == 0, "BB_KMEANS_STATIC_MAX_N must be a power of two");
+constexpr size_t kStaticDoubles = (size_t)kStaticM + 4 * ((size_t)kStaticM + 1);   // = bb_kmeans_workspace_doubles(max n)
+constexpr size_t kStaticInts = (size_t)BB_MAX_LEVELS * (kStaticM + 1);             // = bb_kmeans_workspace_ints(max n, max k)
+constexpr size_t kStaticIntOffset = (kStaticDoubles * sizeof(double) + 255) / 256 * 256;
+constexpr size_t kStaticBytes = kStaticIntOffset + kStaticInts * sizeof(int);
+
+static __device__ __align__(256) unsigned char kmeans_static_scratch[kStaticBytes];
+
+constexpr int kMaxStaticDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[kMaxStaticDevices] = {};   // device address of kmeans_static_scratch, per CUDA ordinal
+
+// true for memory a kernel on the current device can dereference (device or managed allocations)
+bool static_arg_on_device(const void* p) {
+  cudaPointerAttributes a{};
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" int bb_kmeans_levels_static(int device, void* cuda_stream, const double* lambda_dev, int n, int n_levels,
+                                       int log_domain, double* intervals_dev, int ld_int, int* status_dev) {
+  if (!lambda_dev || !intervals_dev || !status_dev || n < 1 || n_levels < 1 || n_levels > BB_MAX_LEVELS || n_levels > n ||
+      ld_int < n_levels || device < 0 || device >= kMaxStaticDevices)
+    return BB_EINVAL;
+  if (n > BB_KMEANS_STATIC_MAX_N) {
+    if (getenv("BB_VERBOSE"))
+      fprintf(stderr, "[bluebild] bb_kmeans_levels_static: n = %d exceeds the static scratch limit of %d eigenvalues; "
+                      "use bb_kmeans_levels (which allocates)\n", n, BB_KMEANS_STATIC_MAX_N);
+    return BB_EUNSUPPORTED;
+  }
+  BB_CUDA(cudaSetDevice(device));
+  if (!static_arg_on_device(lambda_dev) || !static_arg_on_device(intervals_dev) || !static_arg_on_device(status_dev))
+    return BB_EINVAL;                                      // host buffers would need staging memory: not here
+  unsigned char* base = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[device]) {                           // set-up: once per device, with that device current
+      void* p = nullptr;
+      BB_CUDA(cudaGetSymbolAddress(&p, kmeans_static_scratch));
+      g_static_ptr[device] = static_cast<unsigned char*>(p);
+    }
+    base = g_static_ptr[device];
+  }
+  double* ws = reinterpret_cast<double*>(base);
+  int* arg = reinterpret_cast<int*>(base + kStaticIntOffset);
+  return bb_kmeans_levels_dev(lambda_dev, n, n_levels, log_domain != 0, ws, arg, intervals_dev, ld_int, status_dev,
+                              static_cast<cudaStream_t>(cuda_stream));
 }
