@@ -11,8 +11,11 @@
 //   Cholesky-QR (Gram matrix, potrfBatched, trsmBatched), done twice before a Rayleigh-Ritz step.
 // Safety: the residuals |C x - theta x| of the N_eig wanted pairs are computed on the device after each
 // Rayleigh-Ritz step; unless every matrix of the batch meets 1e-11 |theta|_max (or will after a bounded number of
-// further products, estimated from the Ritz values), the caller falls back to the full eigensolve. Indefinite or
-// flat spectra, breakdown of a Cholesky-QR and small problems therefore take the library path, not a wrong answer.
+// further products, estimated from the Ritz values), the caller falls back to the full eigensolve. It also falls
+// back, converged or not, when the block holds a negative Ritz value at least as large in magnitude as the smallest
+// wanted one (powers of C^2 rank by |lambda|, so wanted pairs may then lie outside the block: uniform weighting and
+// other indefinite S). Indefinite or flat spectra, breakdown of a Cholesky-QR and small problems therefore take the
+// library path, not a wrong answer.
 // One host synchronisation of the glue stream per Rayleigh-Ritz step (verdicts of the whole batch in 16 bytes per
 // matrix); the synthesizer stream is not involved.
 #include "glue_internal.h"
@@ -103,9 +106,15 @@ __global__ void verdict_kernel(const double* __restrict__ res2, const double* __
   const double top = fmax(fabs(th[p - 1]), fabs(th[0]));
   const double th_m = th[p - m];                           // the smallest wanted Ritz value
   verdict[2 * b] = top > 0.0 ? sqrt(worst) / top : 0.0;
-  // convergence ratio of the wanted pairs against the block's smallest Ritz value; >= 1 (or a non-positive spectrum
-  // end) means plain powers of C do not separate them
-  verdict[2 * b + 1] = (th_m > 0.0 && th[0] >= 0.0) ? th[0] / th_m : 2.0;
+  // Powers of C^2 find the largest |lambda|, Algorithm 1 l.4 wants the largest lambda. The two agree only while no
+  // negative eigenvalue is as large in magnitude as the smallest wanted one: otherwise the block fills with negative
+  // pairs, wanted positive ones may lie outside it, and small residuals prove nothing (they show that the Ritz pairs
+  // are eigenpairs, not that they are the m largest). th is ascending, so th[0] is the most negative value.
+  // Verdict -1 = "not this solver's problem": the host hands the batch to the full eigensolve whatever the residuals.
+  const bool negative_competes = !(th_m > 0.0) || (th[0] < 0.0 && -th[0] >= th_m);
+  // otherwise: convergence ratio of the wanted pairs against the block's smallest Ritz value; >= 1 (or a slightly
+  // negative spectrum end) means plain powers of C do not separate them
+  verdict[2 * b + 1] = negative_competes ? -1.0 : (th[0] >= 0.0 ? th[0] / th_m : 2.0);
 }
 
 struct Ctx {
@@ -231,7 +240,7 @@ int bb_subspace_top_eigs(GlueWork* g, cudaStream_t st, int nb, int n, int m, Z* 
     int extra = 0;
     for (int b = 0; b < nb; ++b) {
       const double res = w->verdict_host[2 * b], rho = w->verdict_host[2 * b + 1];
-      if (w->info_host[b] != 0 || !(res == res)) { hopeless = true; break; }
+      if (w->info_host[b] != 0 || !(res == res) || rho < 0.0) { hopeless = true; break; }   // rho < 0: indefinite, see verdict_kernel
       if (res <= kResidualTol) continue;
       all = false;
       if (!(rho < 0.95)) { hopeless = true; break; }

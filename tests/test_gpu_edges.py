@@ -259,15 +259,18 @@ def test_one_handle_many_shapes_and_staging_sizes(bb, ctx, oracle, variant):
     assert_parity(s13.images(), ref13, "%s 1x1" % variant)
 
 
-@pytest.mark.parametrize("kind", ["decaying", "flat", "indefinite", "wide_block", "clustered_cut"])
+@pytest.mark.parametrize("kind", ["decaying", "flat", "indefinite", "indefinite_gap", "wide_block", "clustered_cut"])
 def test_eigen_stage_on_every_kind_of_spectrum(bb, ctx, oracle, kind):
     """The glue's leading-eigenpair solver (block subspace iteration, eig_subspace.cu) must either converge or hand
     over to the full batched eigensolve; whichever path runs, eigenvalues and level images must match the oracle:
     a decaying spectrum (the fast path's home ground), a flat one (no separation: fallback), an indefinite one (large
-    negative eigenvalues: powers of C would find those), a block wider than half the matrix (not applicable) and a
-    spectrum with a tight cluster right below the N_eig cut (slow convergence)."""
+    negative eigenvalues: powers of C would find those), the same with a wide gap below the large-magnitude group
+    (10 large positive and 46 large negative eigenvalues fill the 56-wide block and CONVERGE at once, while 14 of the
+    24 wanted pairs are small positive ones outside it: small residuals must not be taken for success), a block wider
+    than half the matrix (not applicable) and a spectrum with a tight cluster right below the N_eig cut (slow
+    convergence)."""
     from paper_2310_09200_b200 import workloads
-    rng = np.random.default_rng({"decaying": 1, "flat": 2, "indefinite": 3, "wide_block": 4, "clustered_cut": 5}[kind])
+    rng = np.random.default_rng({"decaying": 1, "flat": 2, "indefinite": 3, "wide_block": 4, "clustered_cut": 5, "indefinite_gap": 6}[kind])
     n, wl = 288, 2.0
     xyz = np.asfortranarray(np.column_stack([rng.uniform(-400, 400, size=(n, 2)), rng.normal(0, 2, n)]))
     lm = rng.uniform(-0.08, 0.08, size=(300, 2))
@@ -280,6 +283,8 @@ def test_eigen_stage_on_every_kind_of_spectrum(bb, ctx, oracle, kind):
         ev = 1.0 + 1e-3 * rng.random(n)
     elif kind == "indefinite":
         ev = np.concatenate([10.0 ** np.linspace(2, 0, 40), np.full(n - 80, 0.1), -np.linspace(50, 500, 40)])
+    elif kind == "indefinite_gap":
+        ev = np.concatenate([np.linspace(100, 50, 10), 10.0 ** np.linspace(-1, -3, n - 56), -np.linspace(60, 100, 46)])
     elif kind == "wide_block":
         ev = np.concatenate([10.0 ** np.linspace(3, 0, 150), np.full(n - 150, 0.3)])
         n_eig = 100
