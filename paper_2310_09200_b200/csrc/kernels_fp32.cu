@@ -238,11 +238,13 @@ prep_fp32_kernel(PrepArgs a, int KT, int GC, int AC, int n_slabs, int n_chunks, 
   if (tid < 3) cen[tid] = red[tid][0] / (double)a.n_ant;
   __syncthreads();
   // range of the fixed-point phase reduction: |<p', r'>| <= |p'| rmax must stay below 2^19 turns; every block
-  // reaches the same verdict, and a collect that fails it contributes nothing (zero weights) and raises the flag
+  // reaches the same verdict, and a collect that fails it (NaN / Inf coordinates included) contributes nothing
+  // (zero weights, zero B, zero positions) and raises the flag
   double far2 = 0.0;
   for (int i = tid; i < a.n_ant; i += 256) {
     const double dx = a.xyz[i] - cen[0], dy = a.xyz[i + a.ldxyz] - cen[1], dz = a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2];
-    far2 = fmax(far2, dx * dx + dy * dy + dz * dz);
+    const double d2 = dx * dx + dy * dy + dz * dz;
+    if (!(d2 <= far2)) far2 = (d2 == d2) ? d2 : INFINITY;    // fmax would DROP a NaN: a non-finite coordinate must fail the test
   }
   red[0][tid] = far2;
   __syncthreads();
@@ -259,7 +261,7 @@ prep_fp32_kernel(PrepArgs a, int KT, int GC, int AC, int n_slabs, int n_chunks, 
     const int i = (int)(gid / n_eig_pad), k = (int)(gid - (int64_t)i * n_eig_pad);
     double px = 0, py = 0, pz = 0;
     float br = 0.f, bi = 0.f;
-    if (i < a.n_ant) {
+    if (i < a.n_ant && in_range) {                            // a refused collect is packed as zeros: 0 weight x NaN |E|^2 would be NaN
       px = (a.xyz[i] - cen[0]) / a.wavelength;
       py = (a.xyz[i + a.ldxyz] - cen[1]) / a.wavelength;
       pz = (a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2]) / a.wavelength;
@@ -302,8 +304,8 @@ int launch_variant(const Fp32Plan& plan, const SynthArgs& a, cudaStream_t st, in
   auto kern = synth_fp32_kernel<KT, PT, GC, MINB>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + TG * PT - 1) / (TG * PT);
-  const int n_split = a.scratch ? a.n_split : 1;
-  const int cps = (a.n_collects + n_split - 1) / n_split;
+  const int cps = (a.n_collects + (a.scratch ? a.n_split : 1) - 1) / (a.scratch ? a.n_split : 1);
+  const int n_split = (a.n_collects + cps - 1) / cps;      // ranges of cps collects that are not empty (<= a.n_split)
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
     kern<<<dim3((unsigned)tiles, (unsigned)n_split), kThreads, smem, st>>>(a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride,
                                                    (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights,

@@ -678,10 +678,14 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   if (tid < 3) cen[tid] = red[tid][0] / (double)a.n_ant;
   __syncthreads();
   // range of the integer phase reduction: IH = rint(p' 2^8) must fit an int32, i.e. |p'_d| < 2^23 wavelengths; every
-  // block reaches the same verdict, and a collect that fails it contributes nothing (zero weights) and raises the flag
+  // block reaches the same verdict, and a collect that fails it (NaN / Inf coordinates included) contributes nothing
+  // (zero weights, zero B, zero antenna records) and raises the flag
   double far = 0.0;
-  for (int i = tid; i < a.n_ant; i += 256)
-    far = fmax(far, fmax(fabs(a.xyz[i] - cen[0]), fmax(fabs(a.xyz[i + a.ldxyz] - cen[1]), fabs(a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2]))));
+  for (int i = tid; i < a.n_ant; i += 256) {
+    const double dx = fabs(a.xyz[i] - cen[0]), dy = fabs(a.xyz[i + a.ldxyz] - cen[1]), dz = fabs(a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2]);
+    const double d = (dx + dy + dz == dx + dy + dz) ? fmax(dx, fmax(dy, dz)) : INFINITY;   // fmax would DROP a NaN: non-finite input must fail
+    far = fmax(far, d);
+  }
   __shared__ double redm[256];
   redm[tid] = far;
   __syncthreads();
@@ -707,7 +711,7 @@ prep_tc_kernel(PrepArgs a, int NE, int n_chunks, int n_eig_pad, int n_ant_pad, s
   for (int i = tid; i < n_ant_pad; i += 256) {
     double px = 0, py = 0, pz = 0;
     float br = 0.f, bi = 0.f;
-    if (i < a.n_ant) {
+    if (i < a.n_ant && in_range) {                            // a refused collect is packed as zeros: 0 weight x NaN |E|^2 would be NaN
       px = (a.xyz[i] - cen[0]) / a.wavelength;
       py = (a.xyz[i + a.ldxyz] - cen[1]) / a.wavelength;
       pz = (a.xyz[i + 2 * (size_t)a.ldxyz] - cen[2]) / a.wavelength;
@@ -822,8 +826,8 @@ int launch_tc(const TcPlan& plan, const SynthArgs& a, cudaStream_t st, int* laun
   auto kern = synth_tc_kernel<MODE>;
   BB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t tiles = (a.n_pix + kTilePixels - 1) / kTilePixels;
-  const int n_split = a.scratch ? a.n_split : 1;
-  const int cps = (a.n_collects + n_split - 1) / n_split;
+  const int cps = (a.n_collects + (a.scratch ? a.n_split : 1) - 1) / (a.scratch ? a.n_split : 1);
+  const int n_split = (a.n_collects + cps - 1) / cps;      // ranges of cps collects that are not empty (<= a.n_split)
   for (int slab = 0; slab < plan.n_slabs; ++slab) {
     kern<<<dim3((unsigned)tiles, (unsigned)n_split), kThreadsTC, smem, st>>>(
         a.rprime, a.n_pix, a.pix_stride, a.packed, a.packed_stride, (size_t)slab * plan.n_chunks * plan.chunk_bytes, a.weights,
@@ -874,6 +878,10 @@ int bb_collect_split(int64_t tiles, int n_collects, int cta_slots) {
   double best_eff = eff(1);
   for (int s = 2; s <= 8 && n_collects / s >= 4; ++s) {
     if (best_eff >= 0.95) break;
+    // ranges are ceil(n / s) collects long; s such ranges must all be non-empty (25 collects in 6 ranges of 5 would
+    // leave the sixth empty, 33 in 8 ranges of 5 the eighth with a negative length)
+    const int cps = (n_collects + s - 1) / s;
+    if ((s - 1) * cps >= n_collects) continue;
     if (eff(s) > best_eff + 0.05) { best = s; best_eff = eff(s); }
   }
   return best;

@@ -18,9 +18,10 @@ struct bb_uvgrid {
 namespace {
 
 __global__ void density_add_kernel(const double* __restrict__ xyz, int ld, int n_ant, double wavelength, UvGridView g) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x, q = blockIdx.y;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_ant) return;
-  atomicAdd(&g.count[bb_uv_cell(g, xyz, ld, p, q, wavelength)], 1);
+  for (int q = blockIdx.y; q < n_ant; q += gridDim.y)      // gridDim.y is capped at 65535: stride over the second antenna
+    atomicAdd(&g.count[bb_uv_cell(g, xyz, ld, p, q, wavelength)], 1);
 }
 
 }  // namespace
@@ -75,7 +76,7 @@ extern "C" int bb_uvgrid_add(bb_uvgrid* g, int n_ant, double wavelength, const d
   } else {
     BB_CUDA(cudaStreamSynchronize(bb_ctx_user_stream(g->ctx)));   // device input: the caller's work on the context stream is done
   }
-  density_add_kernel<<<dim3((n_ant + 127) / 128, n_ant), 128, 0, st>>>(x, ld, n_ant, wavelength, g->view);
+  density_add_kernel<<<dim3((n_ant + 127) / 128, n_ant < 65535 ? n_ant : 65535), 128, 0, st>>>(x, ld, n_ant, wavelength, g->view);
   BB_CUDA(cudaGetLastError());
   if (!dev) BB_CUDA(cudaStreamSynchronize(st));             // xyz_tmp is reused by the next call
   return BB_OK;

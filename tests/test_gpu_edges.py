@@ -208,6 +208,18 @@ def test_coordinate_range_is_checked_on_the_device(bb, ctx, variant):
         s.get(0, out)
     assert e.value.code == 7
     assert np.array_equal(out, good[0])
+    # NaN / Inf positions must be refused the same way. A maximum taken with fmax() drops a NaN, and a
+    # collect "dropped" by zero weights alone would still add 0 x NaN = NaN to every pixel of every level for good.
+    s.reset()
+    s.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    for bad_value, where in ((np.nan, (3, 1)), (np.inf, (0, 2)), (-np.inf, (11, 0)), (np.nan, (0, 0))):
+        bad = c["xyz"].copy()
+        bad[where] = bad_value
+        s.collect_eig(c["B"], c["D"], np.asfortranarray(bad), c["wavelength"])
+    with pytest.raises(bb.BluebildError) as e:
+        s.get(1, out)
+    assert e.value.code == 7
+    assert np.all(np.isfinite(out)) and np.array_equal(out, good[1])
 
 
 @pytest.mark.parametrize("variant", VARIANTS)

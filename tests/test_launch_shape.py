@@ -34,11 +34,20 @@ def test_split_rules():
         assert 1 <= s <= 8
         if s > 1:
             assert n_col // s >= 4                                   # every range keeps at least 4 collects
+            assert (s - 1) * -(-n_col // s) < n_col, (n_col, s)      # ... and, with ranges of ceil(n / s), the LAST one is not empty
             assert eff(tiles, s, sm) > eff(tiles, 1, sm) + 0.05      # a split must pay
             assert eff(tiles, 1, sm) < 0.95
         if n_col < 8 or eff(tiles, 1, sm) >= 0.95:
             assert s == 1
     assert binding.plan_collect_split("fp16fp8", 0, 64, 16, 2, 10, 148) == 0      # invalid arguments
+    # ranges are ceil(n / s) collects long: 25 collects in 6 ranges of 5, or 33 in 8 ranges of 5, would leave trailing
+    # ranges empty (or of negative length) whose CTAs address weights beyond the queued collects: never chosen
+    for variant in TENSOR + ("fp32",):
+        for n_col in range(1, 129):
+            for n_pix in (256 * 25, 256 * 19, 256 * 37, 256 * 150, 65536, 40000):
+                for sm in (148, 132, 16):
+                    s = binding.plan_collect_split(variant, n_pix, 64, 16, 2, n_col, sm)
+                    assert s >= 1 and (s - 1) * -(-n_col // s) < n_col, (variant, n_col, n_pix, sm, s)
 
 
 def test_nufft_plan_domain_partitioning():
