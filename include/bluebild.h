@@ -247,8 +247,11 @@ int bb_kmeans_levels_static(int device, void* cuda_stream, const double* lambda_
  * device). B, D, xyz: host or device, as bb_synth_collect_eig; the call snapshots them, forms V'_l on the device and
  * STAGES the collect (it synchronises the context stream). The transforms run in bb_nufft_get — ONE set over the
  * baselines of all staged collects, the paper's use of the NUFFT over all time steps — or earlier when 2^24 staged
- * baselines are reached or n_ant changes. BB_EUNSUPPORTED (from the call that runs the transforms; the staged
- * collects are dropped): a pair's fine grids (all levels, complex64) would exceed 32 GB: raise the partition counts.
+ * baselines are reached or n_ant changes. BB_EUNSUPPORTED (from the call that runs the transforms): some pair's fine
+ * grids (all levels, complex64) plus the FFT work area would exceed 32 GB: raise the partition counts. Every pair is
+ * checked, and every buffer and FFT plan is set up, BEFORE the first transform runs, so BB_EUNSUPPORTED and BB_EALLOC
+ * leave the level images exactly as they were (the staged collects are dropped; the handle stays usable). BB_ECUDA from
+ * that call is a launch or execution failure part-way through: the images are then undefined, destroy the handle.
  * Same images as bb_synth_collect_eig up to eps; O(n_ant^2 L w^3 + grid log grid + n_pix L w^3) per pair. */
 typedef struct bb_nufft bb_nufft;
 int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pix, int n_levels, double eps,

@@ -217,7 +217,12 @@ struct bb_nufft {
   std::vector<double> xyz_all, inv_wl_all;      // host: rotated antenna positions [collect][3][n_ant], 1 / wavelength
   double* xyz_all_dev = nullptr; double* inv_wl_dev = nullptr;
   size_t xyz_all_cap = 0, inv_wl_cap = 0;
-  std::map<std::tuple<int, int, int>, cufftHandle> plans;
+  // cuFFT plans per fine-grid shape. They own NO work area (auto-allocation off): all of them run in fft_work, which
+  // is sized before a flush launches anything and counted in the memory limit. Both caches are emptied after a flush
+  // that left them above kMaxCachedPlans / kMaxCachedDec entries.
+  struct FftPlan { cufftHandle handle; size_t work_bytes; };
+  std::map<std::tuple<int, int, int>, FftPlan> plans;
+  unsigned char* fft_work = nullptr; size_t fft_work_cap = 0;
   int64_t n_transforms = 0, max_grid = 0;
 };
 
@@ -354,8 +359,9 @@ extern "C" int bb_nufft_destroy(bb_nufft* h) {
   if (!h) return BB_OK;
   cudaSetDevice(bb_ctx_device(h->ctx));
   cudaStreamSynchronize(bb_ctx_user_stream(h->ctx));
-  for (auto& kv : h->plans) cufftDestroy(kv.second);
+  for (auto& kv : h->plans) cufftDestroy(kv.second.handle);
   for (auto& kv : h->dec) cudaFree(kv.second);
+  cudaFree(h->fft_work);
   cudaFree(h->pix_dev); cudaFree(h->img); cudaFree(h->out_idx_dev); cudaFree(h->V); cudaFree(h->grid); cudaFree(h->fine);
   cudaFree(h->in_idx_dev); cudaFree(h->xyz_all_dev); cudaFree(h->inv_wl_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
   bb_ctx_ref(h->ctx, -1);
@@ -406,18 +412,25 @@ extern "C" int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, in
 
 constexpr int64_t kMaxPendingSources = (int64_t)1 << 24;   // host bookkeeping: 24 B of coordinates + 4 B of index per staged baseline
 
+constexpr size_t kMaxCachedPlans = 64, kMaxCachedDec = 1024;
+
 // One set of transforms over the baselines of all staged collects (Eq. 36 over cells; the sum over time steps is just more sources).
+// Two passes. The first is host-only bookkeeping plus every allocation: the geometry of all (input cell, output cell)
+// pairs, the grid limit, the grids and the shared FFT work area grown to the largest pair, the deconvolution arrays
+// and the cuFFT plans. Whatever can refuse the flush (BB_EUNSUPPORTED, BB_EALLOC, plan creation) does so THERE, before
+// a single kernel has added to the images: the staged collects are dropped, the images are as before the flush. The
+// second pass only launches; an error in it is a CUDA launch or execution failure (BB_ECUDA), after which the images are
+// undefined and the handle should be destroyed.
 static int nufft_flush(bb_nufft* h) {
   if (h->pend == 0) return BB_OK;
   cudaStream_t st = bb_ctx_user_stream(h->ctx);
   const int L = h->n_levels, w = h->kp.w, n_ant = h->pend_n_ant, T = h->pend;
   const int64_t n_base = (int64_t)n_ant * n_ant, n_total = n_base * T;
+  h->pend = 0;                                                          // whatever happens below, the staged collects are consumed
   int rc;
   if ((rc = grow(&h->in_idx_dev, &h->in_idx_cap, (size_t)n_total)) != BB_OK || (rc = grow(&h->xyz_all_dev, &h->xyz_all_cap, h->xyz_all.size())) != BB_OK ||
       (rc = grow(&h->inv_wl_dev, &h->inv_wl_cap, h->inv_wl_all.size())) != BB_OK)
     return rc;
-  BB_CUDA(cudaMemcpyAsync(h->xyz_all_dev, h->xyz_all.data(), h->xyz_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-  BB_CUDA(cudaMemcpyAsync(h->inv_wl_dev, h->inv_wl_all.data(), h->inv_wl_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
   // baselines on the host for the cell bookkeeping (Section 3.4.1): coordinates only, no visibility values
   std::vector<double> bl((size_t)3 * n_total);
   for (int c = 0; c < T; ++c) {
@@ -431,67 +444,104 @@ static int nufft_flush(bb_nufft* h) {
   std::vector<int> in_start, in_order;
   std::vector<double> in_lo, in_hi;
   partition(bl.data(), n_total, n_total, h->n_part_in, in_start, in_order, in_lo, in_hi);
-  BB_CUDA(cudaMemcpyAsync(h->in_idx_dev, in_order.data(), (size_t)n_total * sizeof(int), cudaMemcpyHostToDevice, st));
-  h->pend = 0;
+  const int n_in = h->n_part_in * h->n_part_in, n_out = h->n_part_out * h->n_part_out;
+
+  // ---- pass 1: geometry, limits, allocations, plans -------------------------------------------------
+  struct Pair { int ic, oc; CellGeom g; int64_t n1, n2; const double* dec[3]; bb_nufft::FftPlan* plan; };
+  std::vector<Pair> pairs;
+  int64_t max_n1 = 0, max_n2 = 0;
+  for (int ic = 0; ic < n_in; ++ic) {
+    if (in_start[ic + 1] == in_start[ic]) continue;
+    for (int oc = 0; oc < n_out; ++oc) {
+      if (h->out_start[oc + 1] == h->out_start[oc]) continue;
+      Pair pr{};
+      pr.ic = ic; pr.oc = oc;
+      pair_geometry(&in_lo[ic * 3], &in_hi[ic * 3], &h->out_lo[oc * 3], &h->out_hi[oc * 3], w, pr.g, pr.n1, pr.n2);
+      if ((double)pr.n2 * L * 8.0 > kMaxGridBytes || pr.n2 > 0x7fffffffLL) return BB_EUNSUPPORTED;
+      max_n1 = std::max(max_n1, pr.n1); max_n2 = std::max(max_n2, pr.n2);
+      pairs.push_back(pr);
+    }
+  }
   double gx[kQuad], gw[kQuad];
   gauss_legendre_01(gx, gw);
-  const int n_in = h->n_part_in * h->n_part_in, n_out = h->n_part_out * h->n_part_out;
   std::vector<double> dec;
-  for (int ic = 0; ic < n_in; ++ic) {
-    const int n_src = in_start[ic + 1] - in_start[ic];
-    if (n_src == 0) continue;
-    for (int oc = 0; oc < n_out; ++oc) {
-      const int n_tgt = h->out_start[oc + 1] - h->out_start[oc];
-      if (n_tgt == 0) continue;
-      CellGeom g{};
-      int64_t n1, n2;
-      pair_geometry(&in_lo[ic * 3], &in_hi[ic * 3], &h->out_lo[oc * 3], &h->out_hi[oc * 3], w, g, n1, n2);
-      if ((double)n2 * L * 8.0 > kMaxGridBytes || n2 > 0x7fffffffLL) return BB_EUNSUPPORTED;
-      if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * n2)) != BB_OK)
-        return rc;                                                    // (cudaFree of a buffer in use waits for the device)
-      // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step): one device array per (nf1, nf2), kept
-      const double* decp[3];
-      for (int d = 0; d < 3; ++d) {
-        const auto dk = std::make_pair(g.nf1[d], g.nf2[d]);
-        auto di = h->dec.find(dk);
-        if (di == h->dec.end()) {
-          dec.resize((size_t)g.nf1[d]);
-          for (int i = 0; i < g.nf1[d]; ++i) dec[i] = 1.0 / es_hat_host(6.283185307179586 * (i - g.nf1[d] / 2) / g.nf2[d], h->kp, gx, gw);
-          double* dp = nullptr;
-          if (cudaMalloc(&dp, dec.size() * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
-          BB_CUDA(cudaMemcpy(dp, dec.data(), dec.size() * sizeof(double), cudaMemcpyHostToDevice));
-          di = h->dec.emplace(dk, dp).first;
-        }
-        decp[d] = di->second;
+  size_t work_need = 0;
+  for (Pair& pr : pairs) {
+    // 1 / phihat(2 pi m / nf2) per dimension (Eq. 35 for the inner type-2 step): one device array per (nf1, nf2), kept
+    for (int d = 0; d < 3; ++d) {
+      const auto dk = std::make_pair(pr.g.nf1[d], pr.g.nf2[d]);
+      auto di = h->dec.find(dk);
+      if (di == h->dec.end()) {
+        dec.resize((size_t)pr.g.nf1[d]);
+        for (int i = 0; i < pr.g.nf1[d]; ++i) dec[i] = 1.0 / es_hat_host(6.283185307179586 * (i - pr.g.nf1[d] / 2) / pr.g.nf2[d], h->kp, gx, gw);
+        double* dp = nullptr;
+        if (cudaMalloc(&dp, dec.size() * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return BB_EALLOC; }
+        di = h->dec.emplace(dk, dp).first;                             // owned by the handle from here on
+        BB_CUDA(cudaMemcpy(dp, dec.data(), dec.size() * sizeof(double), cudaMemcpyHostToDevice));
       }
+      pr.dec[d] = di->second;
+    }
+    const auto key = std::make_tuple(pr.g.nf2[0], pr.g.nf2[1], pr.g.nf2[2]);
+    auto it = h->plans.find(key);
+    if (it == h->plans.end()) {
+      bb_nufft::FftPlan fp{};
+      int dims[3] = {pr.g.nf2[2], pr.g.nf2[1], pr.g.nf2[0]};           // slowest first
+      if (cufftCreate(&fp.handle) != CUFFT_SUCCESS) return BB_ECUDA;
+      if (cufftSetAutoAllocation(fp.handle, 0) != CUFFT_SUCCESS ||
+          cufftMakePlanMany(fp.handle, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, 1, &fp.work_bytes) != CUFFT_SUCCESS) {
+        cufftDestroy(fp.handle);
+        return BB_ECUDA;
+      }
+      it = h->plans.emplace(key, fp).first;
+    }
+    pr.plan = &it->second;                                              // std::map: stable under later insertions
+    work_need = std::max(work_need, it->second.work_bytes);
+  }
+  // the FFT work area belongs to the same budget as the fine grids it serves
+  if ((double)max_n2 * L * 8.0 + (double)work_need > kMaxGridBytes) return BB_EUNSUPPORTED;
+  if ((rc = grow(&h->grid, &h->grid_cap, (size_t)L * max_n1)) != BB_OK || (rc = grow(&h->fine, &h->fine_cap, (size_t)L * max_n2)) != BB_OK ||
+      (rc = grow(&h->fft_work, &h->fft_work_cap, std::max(work_need, (size_t)256))) != BB_OK)
+    return rc;                                                          // (cudaFree of a buffer in use waits for the device)
+
+  // ---- pass 2: launches only -----------------------------------------------------------------------
+  auto run = [&]() -> int {
+    BB_CUDA(cudaMemcpyAsync(h->xyz_all_dev, h->xyz_all.data(), h->xyz_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    BB_CUDA(cudaMemcpyAsync(h->inv_wl_dev, h->inv_wl_all.data(), h->inv_wl_all.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    BB_CUDA(cudaMemcpyAsync(h->in_idx_dev, in_order.data(), (size_t)n_total * sizeof(int), cudaMemcpyHostToDevice, st));
+    for (const Pair& pr : pairs) {
+      const int n_src = in_start[pr.ic + 1] - in_start[pr.ic], n_tgt = h->out_start[pr.oc + 1] - h->out_start[pr.oc];
+      const int64_t n1 = pr.n1, n2 = pr.n2;
       BB_CUDA(cudaMemsetAsync(h->grid, 0, (size_t)L * n1 * sizeof(float2), st));
       BB_CUDA(cudaMemsetAsync(h->fine, 0, (size_t)L * n2 * sizeof(float2), st));
-      spread_kernel<<<(unsigned)((n_src + 3) / 4), 128, 0, st>>>(h->in_idx_dev + in_start[ic], n_src, h->xyz_all_dev, n_ant, h->inv_wl_dev,
-                                                                    h->V, L, g, h->kp, h->grid);
+      spread_kernel<<<(unsigned)((n_src + 3) / 4), 128, 0, st>>>(h->in_idx_dev + in_start[pr.ic], n_src, h->xyz_all_dev, n_ant, h->inv_wl_dev,
+                                                                    h->V, L, pr.g, h->kp, h->grid);
       BB_CUDA(cudaGetLastError());
-      deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, g, decp[0], decp[1], decp[2], h->fine);
+      deconv_pad_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>(h->grid, L, pr.g, pr.dec[0], pr.dec[1], pr.dec[2], h->fine);
       BB_CUDA(cudaGetLastError());
-      const auto key = std::make_tuple(g.nf2[0], g.nf2[1], g.nf2[2]);
-      auto it = h->plans.find(key);
-      if (it == h->plans.end()) {
-        cufftHandle plan;
-        int dims[3] = {g.nf2[2], g.nf2[1], g.nf2[0]};                 // slowest first
-        if (cufftPlanMany(&plan, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, 1) != CUFFT_SUCCESS) return BB_ECUDA;
-        it = h->plans.emplace(key, plan).first;
-      }
-      if (cufftSetStream(it->second, st) != CUFFT_SUCCESS) return BB_ECUDA;
+      if (cufftSetStream(pr.plan->handle, st) != CUFFT_SUCCESS || cufftSetWorkArea(pr.plan->handle, h->fft_work) != CUFFT_SUCCESS) return BB_ECUDA;
       for (int l = 0; l < L; ++l)                                      // u_k = sum_m b_m exp(+i m k h2): the unnormalised inverse
-        if (cufftExecC2C(it->second, reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2),
+        if (cufftExecC2C(pr.plan->handle, reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2),
                          reinterpret_cast<cufftComplex*>(h->fine + (size_t)l * n2), CUFFT_INVERSE) != CUFFT_SUCCESS) return BB_ECUDA;
-      interp_kernel<<<(unsigned)((n_tgt + 3) / 4), 128, 0, st>>>(h->out_idx_dev + h->out_start[oc], n_tgt, h->pix_dev, h->n_pix,
-                                                                    h->fine, L, g, h->kp, h->img, h->pix_stride);
+      interp_kernel<<<(unsigned)((n_tgt + 3) / 4), 128, 0, st>>>(h->out_idx_dev + h->out_start[pr.oc], n_tgt, h->pix_dev, h->n_pix,
+                                                                    h->fine, L, pr.g, h->kp, h->img, h->pix_stride);
       BB_CUDA(cudaGetLastError());
       h->n_transforms += 1;
       h->max_grid = std::max(h->max_grid, n2);
     }
+    return BB_OK;
+  };
+  rc = run();
+  const cudaError_t e = cudaStreamSynchronize(st);                      // on every path: host vectors above are in flight until here
+  if (rc == BB_OK && e != cudaSuccess) { bb_note_cuda_error(e, "bb_nufft flush", __FILE__, __LINE__); rc = BB_ECUDA; }
+  if (h->plans.size() > kMaxCachedPlans) {
+    for (auto& kv : h->plans) cufftDestroy(kv.second.handle);
+    h->plans.clear();
   }
-  BB_CUDA(cudaStreamSynchronize(st));
-  return BB_OK;
+  if (h->dec.size() > kMaxCachedDec) {
+    for (auto& kv : h->dec) cudaFree(kv.second);
+    h->dec.clear();
+  }
+  return rc;
 }
 
 extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,

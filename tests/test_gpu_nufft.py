@@ -111,6 +111,30 @@ def test_argument_validation_and_grid_limit(bb, ctx):
     assert e.value.code == 7                                                # BB_EUNSUPPORTED: raise the partition counts
 
 
+def test_a_refused_flush_leaves_the_images_untouched(bb, ctx):
+    """the grid limit is checked for ALL (input cell, output cell) pairs before any of them is transformed. Seven
+    antennas within 50 m and one 570 km away, 2 x 2 input cells: the cells that hold only short baselines need tiny grids,
+    the two that also hold the long ones exceed the limit. Whatever the order of the cells, a refused bb_nufft_get must not
+    have run a single transform: the images are those of the earlier, good collect, bit for bit, and stay usable."""
+    c = case(51, 8, 4, 2, 8, 50.0, np.deg2rad(40.0))
+    h = bb.NufftSynthesis(ctx, c["pix"], 2, eps=1e-6, n_part_in=2, n_part_out=1)
+    h.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])
+    good = h.images().copy()
+    assert np.max(np.abs(good)) > 0
+    for direction in ((1, 1, 0), (1, -1, 0), (1, 0, 1), (0, 1, -1), (1, 1, 1), (-1, 1, 1)):
+        before = h.stats()["n_transforms"]
+        far = c["xyz"].copy()
+        far[7] += 4.0e5 * np.array(direction, dtype=np.float64)
+        h.collect_eig(c["B"], c["D"], np.asfortranarray(far), c["wavelength"])     # staged only
+        with pytest.raises(bb.BluebildError) as e:
+            h.images()
+        assert e.value.code == 7
+        assert h.stats()["n_transforms"] == before, direction                     # no pair ran
+        assert np.array_equal(h.images(), good), direction                         # staged collect dropped, images as before
+    h.collect_eig(c["B"], c["D"], c["xyz"], c["wavelength"])                        # and the handle still works
+    assert np.allclose(h.images(), 2 * good, rtol=1e-5, atol=1e-6 * np.max(np.abs(good)))
+
+
 def test_staging_flushes_when_the_array_changes(bb, ctx, oracle):
     """Staged collects share one source list only while n_ant stays the same: a different array runs the pending transforms first."""
     ca = case(41, 12, 5, 2, 24, 300.0, np.deg2rad(8.0))
