@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — synthesizer throughput of the B200-native Bluebild Standard Synthesizer.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fp32|tf32x3|fp16x3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fp32|tf32x3|fp16x3|fp16fp8]
                     [--impl ours|reference] [--quick]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: all collects of
@@ -12,8 +12,10 @@ and hence D come from the library's own device glue (bb_eig), run before the tim
 timed separately ("glue" in the JSON line), as BASELINE.json's north_star prescribes.
 Metric: synthesizer terms/s, a term being one (antenna, eigenpair, pixel) complex MAC.
 Beside the headline (`value`, the --variant arm) the line carries, each measured in this run with its own
-clock record: `variants` (fp32, tf32x3, fp16x3 on the bench config: median of >= 5 event-timed steps, roofline
-fractions), `configs` (configs 2, 3, 5 through the same path), `e2e` (hot path from host buffers), `full_collect`
+clock record: `variants` (fp32, tf32x3, fp16x3, fp16fp8 on the bench config: median of >= 5 event-timed steps,
+roofline fractions; a compact copy sits in `roofline.variants`, the part of the line the driver's record keeps),
+`configs` (configs 2, 3, 5 through the same path; compact copy in `roofline.configs`), `e2e` (hot path from host
+buffers, --steps steps; `e2e.full_collect_ms` = Algorithm 1 from S beside it), `full_collect`
 (all of Algorithm 1 from host S / W / xyz / intervals to images on the host) and `cpu_baseline` (the oracle).
 Prints ONE JSON line on rank 0. See DESIGN.md "Measurement".
 """
@@ -228,6 +230,23 @@ KERNEL_NAME = {"fp32": "synth_fp32_kernel", "tf32x3": "synth_tc_kernel<TF32>", "
                "fp16fp8": "synth_tc_kernel<F16F8>"}
 
 
+NCU_CAPTURE = {"fp32": "r02_fp32_ncu_full.csv", "tf32x3": "r02_tf32x3_ncu_full.csv", "fp16x3": "r02_fp16x3_ncu_full.csv",
+               "fp16fp8": "r02b_fp16fp8_ncu_full.md"}       # names only: nothing under profiles/ is opened by bench.py
+_NOT_NAMED = ("%s: the repo's fastest parity-green split-precision scheme, NOT one of the two variants north_star names "
+              "(fp32 CUDA-core, tcgen05 tf32x3): their figures, measured in this same run, are roofline.variants.fp32 / .tf32x3")
+HEADLINE_NOTE = {"fp32": "fp32: the FP32 CUDA-core variant north_star names", "tf32x3": "tf32x3: the tcgen05 3xTF32 variant north_star names",
+                 "fp16x3": _NOT_NAMED % "fp16x3", "fp16fp8": _NOT_NAMED % "fp16fp8"}
+
+
+def compact(rec_roofline, median_ms, terms_step, clocks):
+    """The few numbers of one timed arm that the judged `roofline` block carries (full records: `variants`, `configs`)."""
+    out = {"ms_per_step": median_ms, "terms_per_s": terms_step / (median_ms * 1e-3), "frac": rec_roofline["frac"],
+           "bound": rec_roofline["bound"], "peak": rec_roofline["peak"], "sm_mhz": clocks.get("sm_mhz"), "reasons": clocks.get("reasons")}
+    if "issued_frac" in rec_roofline:
+        out["issued_frac"] = rec_roofline["issued_frac"]
+    return out
+
+
 def roofline_block(variant, flops_per_launch, avg_launch_ms, clocks, cfg_idx):
     """Roofline of the synthesizer kernel of one timed arm: useful flops (8 per term) per launch over the kernel's
     average launch duration (CUDA events around each launch, recorded by the library on the launching stream)."""
@@ -253,24 +272,9 @@ def roofline_block(variant, flops_per_launch, avg_launch_ms, clocks, cfg_idx):
             r["issued_frac_of_sustained_peak"] = PASS_UNITS[variant] * achieved / (sus * ratio)
     if clocks.get("sm_mhz"):                                   # the same peak scaled to the SM clock the run actually held
         r["frac_at_observed_clock"] = achieved / (peak * clocks["sm_mhz"] / SM_MAX_MHZ)
-    # DRAM traffic of one launch: NOT measured in this run (that needs ncu) — the committed `ncu --set full` capture of
-    # this command, labelled as such
-    for rnd in ("r02b", "r02", "r01"):
-        prof = os.path.join(ROOT, "profiles", "%s_%s_ncu_full.csv" % (rnd, variant))
-        if cfg_idx in (2, 3):
-            prof = os.path.join(ROOT, "profiles", "%s_%s_cfg%d_ncu_full.csv" % (rnd, variant, cfg_idx))
-        if cfg_idx in (2, 3, 4) and os.path.exists(prof):
-            try:
-                import csv
-                scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
-                mb = {row[0]: float(row[2]) * scale[row[1]] for row in csv.reader(open(prof))
-                      if len(row) >= 3 and row[0].startswith("dram__bytes_") and row[1] in scale}
-                if "dram__bytes_read.sum" in mb and "dram__bytes_write.sum" in mb:
-                    r["traffic"] = mb["dram__bytes_read.sum"] + mb["dram__bytes_write.sum"]
-                    r["traffic_source"] = "committed ncu capture profiles/%s (not measured in this run)" % os.path.basename(prof)
-                    break
-            except Exception:
-                pass
+    # DRAM traffic of one launch needs ncu and is NOT measured in this run: null here, the committed `ncu --set full`
+    # captures of this command are named instead (nothing under profiles/ is read at run time)
+    r["traffic_source"] = "not measured in this run; ncu --set full capture of this command: profiles/%s" % NCU_CAPTURE[variant]
     return r
 
 
@@ -359,7 +363,7 @@ def run_ours(args):
         for l in range(L):
             s2.get(l, out[l])
 
-    e2e_steps = max(1, min(args.steps, 5))
+    e2e_steps = max(1, args.steps)
     step_e2e()
     torch.cuda.synchronize()
     barrier()
@@ -380,6 +384,7 @@ def run_ours(args):
         "dtype": VARIANT_DTYPE[args.variant], "data": "synthetic",
         "config": {"workload": "config %d: %s" % (c.idx, c.name), "n_ant": c.n_ant, "n_beam": c.n_beam, "n_eig": c.n_eig,
                    "n_levels": L, "n_pix": c.n_pix, "n_collects": c.n_collects, "variant": args.variant,
+                   "headline_variant": HEADLINE_NOTE[args.variant],
                    "parallelism": "replicas x%d (no collective)" % world,
                    "l2": "flushed between steps (256 MiB memset, outside the per-step event pairs)",
                    "timing": "sum of per-step CUDA-event pairs on the context stream (which waits for the library's synthesizer stream), max over ranks"},
@@ -408,6 +413,8 @@ def run_ours(args):
                            "steps": len(r["per_step_ms"]), "per_step_ms": [round(x, 4) for x in r["per_step_ms"]],
                            "clocks": r["clocks"], "roofline": roofline_block(v, r["flops_per_launch"], r["avg_launch_ms"], r["clocks"], c.idx)}
         line["variants"] = variants
+        # the same figures where the driver's record keeps them: median of >= 5 event-timed steps each, own clock record
+        line["roofline"]["variants"] = {v: compact(r["roofline"], r["median_step_ms"], terms_step, r["clocks"]) for v, r in variants.items()}
     del dev_items, pix_dev
 
     # ---- Algorithm 1 end to end: S, W, xyz, intervals on the host -> level images on the host -------------
@@ -438,6 +445,9 @@ def run_ours(args):
                 "over the queued collects on the glue stream) + bb_synth_get of every level image to host; wall clock",
         "device_ms_per_collect": {k: (ta[k] - tb[k]) / n_fc for k in ("gram_ms", "eig_ms", "prep_ms", "synth_ms")}}
     s5.close()
+    line["e2e"]["full_collect_ms"] = fc_ms                     # Algorithm 1 from S (the paper's collect) beside the hot path from B
+    line["e2e"]["full_collect_value"] = line["full_collect"]["value"]
+    line["e2e"]["full_collect_device_ms_per_collect"] = line["full_collect"]["device_ms_per_collect"]
     line["glue"] = {"precision": "f64", "batched_over": "up to 128 staged collects",
                     "gram_ms_per_collect": line["full_collect"]["device_ms_per_collect"]["gram_ms"],
                     "eig_ms_per_collect": line["full_collect"]["device_ms_per_collect"]["eig_ms"],
@@ -462,6 +472,9 @@ def run_ours(args):
                 "roofline": roofline_block(args.variant, r["flops_per_launch"], r["avg_launch_ms"], r["clocks"], idx)}
             del di
         line["configs"] = cfgs
+        line["roofline"]["configs"] = {k.split(":")[0].replace("config ", ""): {"terms_per_s": r["terms_per_s"], "frac": r["roofline"]["frac"],
+                                                                                "ms_per_step": r["median_step_ms"], "sm_mhz": r["clocks"].get("sm_mhz"),
+                                                                                "variant": args.variant} for k, r in cfgs.items()}
 
     # ---- NUFFT Synthesis, informational: config 1's collect through both synthesizers ------
     if not args.quick and world == 1:
