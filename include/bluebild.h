@@ -136,7 +136,19 @@ int bb_synth_collect_batch(bb_synth* s, int n_collects, int n_ant, int n_beam, i
  * Coordinate range of the phase generator, with p' = (xyz - mean(xyz)) / wavelength and r' the pixel vectors
  * minus the centre of their bounding box: FP32 variant |p'| max|r'| < 2^19 turns; tensor variants
  * |p'_x|, |p'_y|, |p'_z| < 2^23 wavelengths. Checked on the device: a collect beyond it contributes nothing
- * and bb_synth_get / bb_synth_status return BB_EUNSUPPORTED. */
+ * and bb_synth_get / bb_synth_status return BB_EUNSUPPORTED.
+ * Antenna-count limit of the tensor variants (every collect call; checked on the host, the call returns
+ * BB_EUNSUPPORTED with nothing queued and the images unchanged): n_ant <= BB_MAX_ANT_TF32X3 / _FP16X3 / _FP16_FP8.
+ * Reason: each tcgen05.mma that adds into the fp32 accumulator drops a fraction of an ulp, always towards zero, so
+ * these variants' images are too small by a factor that grows with the number of instructions per accumulator,
+ * n_ant / 16 x {12, 6, 4}: measured -2.45e-8, -1.24e-8, -0.82e-8 per antenna on one B200, i.e. -4.4e-5 for tf32x3 at
+ * the 1776 antennas of BASELINE config 2 and -2.0e-4, twice the 1e-4 tolerance, at 8192 (profiles/r03_n_ant_bias.md).
+ * The limits keep that shrink at or below 5.1e-5, half the tolerance, because the constant depends on how the sum
+ * grows (up to 1.5x for an array whose first antennas dominate). The FP32 variant has no such term (n_ant <= 2^20):
+ * arrays beamformed from more elements (Eq. 22-24) go through BB_VARIANT_FP32. */
+#define BB_MAX_ANT_TF32X3 2048
+#define BB_MAX_ANT_FP16X3 4096
+#define BB_MAX_ANT_FP16_FP8 6144
 int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wavelength, const bb_c32* B,
                          int ldb, const float* D, int ldd, const double* xyz, int ldxyz);
 

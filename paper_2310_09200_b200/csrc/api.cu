@@ -449,11 +449,24 @@ static int enqueue_prepared(bb_synth* s, int n_ant, int n_eig, double wavelength
   return BB_OK;
 }
 
+// Largest antenna count a variant takes (include/bluebild.h "Antenna-count limit"): the tensor variants' fp32
+// accumulator loses a fraction of an ulp, always towards zero, with every tcgen05.mma that adds to it, so their images
+// come out too small by a factor that grows with n_ant / 16 x {12, 6, 4} instructions (measured: profiles/r03_n_ant_bias.md).
+static int max_antennas(int variant) {
+  switch (variant) {
+    case BB_VARIANT_TF32X3: return BB_MAX_ANT_TF32X3;
+    case BB_VARIANT_FP16X3: return BB_MAX_ANT_FP16X3;
+    case BB_VARIANT_FP16_FP8: return BB_MAX_ANT_FP16_FP8;
+    default: return 1 << 20;
+  }
+}
+
 extern "C" int bb_synth_collect_eig(bb_synth* s, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
                                     const float* D, int ldd, const double* xyz, int ldxyz) {
   if (!s || !B || !D || !xyz || n_ant < 1 || n_eig < 1 || !(wavelength > 0.0) || ldb < n_ant ||
       ldd < s->n_levels || ldxyz < n_ant || n_eig > 4096 || n_ant > (1 << 20))
     return BB_EINVAL;
+  if (n_ant > max_antennas(s->variant)) return BB_EUNSUPPORTED;    // nothing queued, images unchanged: use BB_VARIANT_FP32
   BB_CUDA(cudaSetDevice(s->ctx->device));
   const int L = s->n_levels;
   const size_t need = up16((size_t)n_ant * n_eig * 8) + up16((size_t)L * n_eig * 4) + up16((size_t)n_ant * 24);
@@ -612,6 +625,7 @@ static int check_full_args(bb_synth* s, int n_ant, int n_beam, int n_eig, double
   if (n_ant < 1 || n_beam < 1 || n_eig < 1 || n_eig > n_beam || n_beam > BB_MAX_BEAMS || !(wavelength > 0.0) || lds < n_beam ||
       ldxyz < n_ant || ld_int < n_intervals || (W && ldw < n_ant) || (!W && n_beam != n_ant) || n_ant > (1 << 20))
     return BB_EINVAL;
+  if (n_ant > max_antennas(s->variant)) return BB_EUNSUPPORTED;    // nothing staged, images unchanged: use BB_VARIANT_FP32
   return BB_OK;
 }
 

@@ -222,6 +222,51 @@ def test_coordinate_range_is_checked_on_the_device(bb, ctx, variant):
     assert np.all(np.isfinite(out)) and np.array_equal(out, good[1])
 
 
+MAX_ANT = {"fp32": 1 << 20, "tf32x3": 2048, "fp16x3": 4096, "fp16fp8": 6144}     # include/bluebild.h BB_MAX_ANT_*
+
+
+@pytest.mark.parametrize("n_ant", [2048, 4096, 6144, 8192])
+def test_antenna_count_limit_of_the_tensor_variants(bb, ctx, oracle, n_ant):
+    """VERDICT r2 item 2. The tensor variants' images shrink by a factor that grows with the antenna count (every
+    tcgen05.mma truncates the fp32 accumulator), which no BASELINE config shows (largest: 1776). Each variant must
+    either meet the tolerance or refuse the call: at its documented limit it is measured against the oracle (rel-L2,
+    max-abs / peak and the fitted scale got / ref per level are recorded), beyond it collect_eig and collect return
+    BB_EUNSUPPORTED and leave the images alone. One collect, N_eig 16 in 2 levels, 2048 random pixels."""
+    from helpers import record_parity
+    rng = np.random.default_rng(n_ant)
+    n_eig, L, n_pix = 16, 2, 2048
+    B = np.asfortranarray(((rng.normal(size=(n_ant, n_eig)) + 1j * rng.normal(size=(n_ant, n_eig))) / np.sqrt(n_ant)).astype(np.complex64))
+    D = np.zeros((L, n_eig), np.float32)
+    D[0, :8] = rng.uniform(0.5, 3, 8)
+    D[1, 8:] = rng.uniform(0.5, 3, 8)
+    D = np.asfortranarray(D)
+    xyz = np.asfortranarray(rng.uniform(-3000, 3000, size=(n_ant, 3)) * np.array([1, 1, 0.01]) + np.array([6.1e6, -2.3e5, 1.7e6]))
+    lm = rng.uniform(-0.2, 0.2, size=(n_pix, 2))
+    pix = np.asfortranarray(np.column_stack([lm, np.sqrt(1 - np.sum(lm * lm, axis=1))]))
+    ref = oracle.synth(B, D, xyz, pix, 2.7)
+    for variant in VARIANTS:
+        s = bb.StandardSynthesis(ctx, pix, L, variant)
+        if n_ant <= MAX_ANT[variant]:
+            s.collect_eig(B, D, xyz, 2.7)
+            got = s.images().astype(np.float64)
+            nums = record_parity("n_ant %d" % n_ant, "antenna-count limit", variant, got, ref, 1, n_pix)
+            scale = [float(np.dot(got[l], ref[l]) / np.dot(ref[l], ref[l])) - 1.0 for l in range(L)]
+            print("n_ant %d %s: rel-L2 %s max-abs/peak %s fitted scale - 1 %s" % (
+                n_ant, variant, ["%.2e" % a for a, _ in nums], ["%.2e" % b for _, b in nums], ["%+.2e" % x for x in scale]))
+            assert_parity(got, ref, "%s at %d antennas" % (variant, n_ant))
+            if variant != "fp32":
+                assert all(-6.5e-5 < x < 0.0 for x in scale), (variant, scale)      # a shrink, inside the bound the header states
+        else:
+            with pytest.raises(bb.BluebildError) as e:
+                s.collect_eig(B, D, xyz, 2.7)
+            assert e.value.code == 7
+            with pytest.raises(bb.BluebildError) as e:                           # Algorithm 1 entry: refused before anything is staged
+                s.collect(np.eye(4, dtype=np.complex64), np.ones((n_ant, 4), dtype=np.complex64), xyz, 2.7, 2, np.array([[0.0, 1e30], [-1e30, 0.0]]))
+            assert e.value.code == 7
+            assert np.all(s.images() == 0.0)
+        s.close()
+
+
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_one_handle_many_shapes_and_staging_sizes(bb, ctx, oracle, variant):
     """the staging slot must follow what each call stages. collect_eig (small slots) then collect
