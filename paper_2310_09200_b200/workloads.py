@@ -215,12 +215,18 @@ class Workload:
     def mid_collect(self) -> int:
         return (self.cfg.n_epochs // 2) * self.cfg.n_chan
 
-    def sample_pixels(self, stride: int = 16) -> np.ndarray:
+    def sample_pixels(self, stride: int = 16, full_tiles: bool = False) -> np.ndarray:
         """Deterministic pixel subset: every stride-th row and column + pixel nearest each of the
-        10 brightest sources (pixels are independent, so a subset image is exact for them)."""
+        10 brightest sources (pixels are independent, so a subset image is exact for them).
+        full_tiles: also 1024 CONSECUTIVE pixels from a 256-aligned index near the image centre and the last 256
+        pixels of the image. A strided grid only ever lands on pixel indices that are multiples of the stride; a
+        kernel that maps consecutive pixels to the threads (lanes) of a tile is then compared on a few lanes only."""
         n = self.cfg.n_side
         rows = np.arange(0, n, stride)
         idx = (rows[None, :] + n * rows[:, None]).ravel()
+        if full_tiles:
+            start = ((n * n // 2 + n // 3) // 256) * 256
+            idx = np.concatenate([idx, np.arange(start, min(start + 1024, n * n)), np.arange(max(n * n - 256, 0), n * n)])
         g0 = -(n // 2) * self.pix_step
         bright = np.argsort(self.src_flux)[::-1][:10]
         a = np.clip(np.rint((self.src_lm[bright, 0] - g0) / self.pix_step), 0, n - 1).astype(np.int64)

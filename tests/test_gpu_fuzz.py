@@ -15,9 +15,12 @@ def test_random_shapes_agree_across_variants_and_runs(oracle):
     ctx = binding.Context(0)
     rng = np.random.default_rng(20231009)
     worst = 0.0
-    for case in range(120):
+    for case in range(126):
         n_ant = int(rng.integers(1, 200)); n_eig = int(rng.integers(1, 140)); L = int(rng.integers(1, 12))
         n_pix = int(rng.integers(1, 3000)); n_col = int(rng.integers(1, 40))
+        big = case >= 120                       # six large arrays (up to ~2000 antennas, the tf32x3 limit is 2048), few collects
+        if big:
+            n_ant = int(rng.integers(200, 2000)); n_col = int(rng.integers(1, 5))
         fov = rng.uniform(0.01, 0.6); ext = 10 ** rng.uniform(1, 4.5); wl = rng.uniform(0.5, 10)
         lm = rng.uniform(-fov, fov, size=(n_pix, 2))
         pix = np.asfortranarray(np.column_stack([lm, np.sqrt(1 - np.sum(lm * lm, axis=1))]))
@@ -45,9 +48,10 @@ def test_random_shapes_agree_across_variants_and_runs(oracle):
             oracle.synth(B, D, xyz, np.asfortranarray(pix[sub]), wl, img=ref_o)
         for v in imgs:
             err_o = np.max(np.abs(imgs[v][:, sub] - ref_o)) / (np.max(np.abs(ref_o)) or 1.0)
-            assert err_o < (2e-6 if v == "fp32" else 1e-4), ("vs oracle", v, err_o, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
+            assert err_o < ((5e-6 if big else 2e-6) if v == "fp32" else 1e-4), ("vs oracle", v, err_o, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
         for v in ("fp16x3", "tf32x3", "fp16fp8"):
             err = np.max(np.abs(imgs[v] - ref)) / peak
             worst = max(worst, err)
-            assert err < 5e-5, (v, err, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
+            # large arrays: the tensor variants' antenna-count shrink (<= 5.1e-5 at their limits, include/bluebild.h) adds to it
+            assert err < (1e-4 if big else 5e-5), (v, err, n_ant, n_eig, L, n_pix, n_col, ext, wl, fov)
     print("worst max-abs / peak between variants: %.2e" % worst)

@@ -82,7 +82,7 @@ def test_cfg1_full_collect_with_device_glue(bb, ctx, wl, oracle, variant):
 
 # ------------------------------------------------------------------------------------ configs 2-5, ALL collects
 # SURVEY 8(d) "Oracle timing beside it": full image for config 2, the every-8th / every-16th pixel subset
-# (+ the pixels nearest the 10 brightest sources) for configs 3, 4 and 5 — over EVERY collect of the config, because
+# (+ the pixels nearest the 10 brightest sources + 1280 consecutive pixels: whole tiles) for configs 3, 4 and 5 — over EVERY collect of the config, because
 # every time step and band accumulates into the same images. The oracle side (eigen stage of
 # each collect, then Alg. 2) is computed once per config and shared by the three variants.
 _FULL = {2: dict(stride=None), 3: dict(stride=8), 4: dict(stride=16), 5: dict(stride=16)}
@@ -101,7 +101,8 @@ def oracle_case(oracle, wl, cfg_idx):
     assert_well_posed(items, iv)
     attach_weights(oracle, items, iv)
     stride = _FULL[cfg_idx]["stride"]
-    sub = None if stride is None else w.sample_pixels(stride)
+    # + four whole consecutive 256-pixel tiles and the image's last tile: every thread / TMEM lane of a tile at full size
+    sub = None if stride is None else w.sample_pixels(stride, full_tiles=True)
     ref = oracle_images(oracle, items, w.pixels(sub), c.n_levels)
     _cache[cfg_idx] = dict(w=w, items=items, iv=iv, sub=sub, ref=ref)
     return _cache[cfg_idx]
@@ -126,7 +127,8 @@ def test_G1_all_collects(bb, ctx, wl, oracle, cfg_idx, variant):
     s.close()
 
 
-_G2_COLLECTS = {2: None, 3: None, 4: None, 5: [n for t in (0, 24, 49) for n in range(t * 16, t * 16 + 16)]}
+# config 5: 9 epochs x 16 channels = 144 collects = one FULL glue group of 128 staged collects + a partial one of 16
+_G2_COLLECTS = {2: None, 3: None, 4: None, 5: [n for t in (0, 6, 12, 18, 24, 30, 36, 42, 49) for n in range(t * 16, t * 16 + 16)]}
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -135,7 +137,7 @@ _G2_COLLECTS = {2: None, 3: None, 4: None, 5: [n for t in (0, 24, 49) for n in r
 def test_G2_device_glue(bb, ctx, wl, oracle, cfg_idx, api, variant):
     """Algorithm 1 end to end on the device (batched fp64 Gram / Cholesky / eigensolve, level weights, hot path)
     from S, W, xyz and the intervals, through bb_synth_collect and bb_synth_collect_batch, on the oracle's pixel
-    subset: all collects of configs 2-4, 3 epochs x 16 channels of config 5."""
+    subset: all collects of configs 2-4, 9 epochs x 16 channels of config 5 (a full 128-collect glue group and a partial one)."""
     from helpers import record_parity
     case = oracle_case(oracle, wl, cfg_idx)
     w, iv, sub = case["w"], case["iv"], case["sub"]

@@ -33,6 +33,12 @@ def test_pixel_grid_unit_vectors_and_centre():
     assert np.allclose(pix[centre], w.r_c, atol=1e-15)                     # a pixel sits on r_c
     sub = w.sample_pixels(16)
     assert sub.size >= 32 * 32 and np.all(np.diff(sub) > 0)
+    full = w.sample_pixels(16, full_tiles=True)
+    assert np.all(np.diff(full) > 0) and np.all(np.isin(sub, full)) and full[-1] == 512 * 512 - 1
+    runs = np.split(full, np.where(np.diff(full) != 1)[0] + 1)
+    longest = max(runs, key=len)
+    assert len(longest) >= 1024 and longest[0] % 256 == 0            # four whole 256-pixel tiles, tile-aligned
+    assert set(full[-256:] % 256) == set(range(256))                 # the last tile: every lane
 
 
 def test_earth_rotation_preserves_geometry():
