@@ -271,6 +271,14 @@ int bb_nufft_create(bb_ctx* ctx, int64_t n_pix, const double* pix, int64_t ld_pi
 int bb_nufft_destroy(bb_nufft* h);
 int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wavelength, const bb_c32* B, int ldb,
                          const float* D, int ldd, const double* xyz, int ldxyz);
+/* Algorithm 3 from its own inputs: Gram matrix, generalized eigendecomposition, N_eig largest pairs
+ * (l.2-4), interval selection and filters (l.5-7), V per level and the NUFFT (l.8-9). Arguments as bb_synth_collect_ex
+ * (sinc Gram); the handle's n_levels must equal n_intervals * n_filters, image index = filter * n_intervals + interval.
+ * n_ant <= 4096, n_beam <= BB_MAX_BEAMS. Synchronous up to the staging: BB_ENOTPOSDEF / BB_ENOCONV are returned by this
+ * call and nothing is staged. Same images as bb_synth_collect_ex up to eps. */
+int bb_nufft_collect(bb_nufft* h, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W, int ldw,
+                     const bb_c32* S, int lds, const double* xyz, int ldxyz, const double* intervals, int ld_int,
+                     int n_filters, const int* filters);
 int bb_nufft_get(bb_nufft* h, int level, float* out);   /* n_pix floats, host or device; synchronises */
 /* number of transforms run and the largest fine grid (points) so far: what Section 3.4.1 / Figure 1c is about */
 int bb_nufft_stats(bb_nufft* h, int64_t* n_transforms, int64_t* max_grid_points);

@@ -29,7 +29,7 @@ EXPORTS = ["bb_ctx_create", "bb_ctx_destroy", "bb_synth_create", "bb_synth_destr
            "bb_synth_collect", "bb_synth_collect_ex", "bb_synth_collect_batch", "bb_synth_collect_eig", "bb_synth_flush", "bb_synth_get", "bb_synth_timings",
            "bb_synth_status", "bb_synth_launches", "bb_eig", "bb_level_weights", "bb_uvgrid_create", "bb_uvgrid_add",
            "bb_uvgrid_destroy", "bb_synth_set_weighting", "bb_estimate_n_eig", "bb_kmeans_levels", "bb_kmeans_levels_static", "bb_status_string", "bb_version",
-           "bb_plan_collect_split", "bb_nufft_plan", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_get", "bb_nufft_stats"]
+           "bb_plan_collect_split", "bb_nufft_plan", "bb_nufft_create", "bb_nufft_destroy", "bb_nufft_collect_eig", "bb_nufft_collect", "bb_nufft_get", "bb_nufft_stats"]
 
 _lib = None
 
@@ -82,6 +82,7 @@ def load_library(path: str = LIB_PATH):
         "bb_nufft_create": ([vp, i64, vp, i64, i32, f64, i32, i32, pp], i32),
         "bb_nufft_destroy": ([vp], i32),
         "bb_nufft_collect_eig": ([vp, i32, i32, f64, vp, i32, vp, i32, vp, i32], i32),
+        "bb_nufft_collect": ([vp, i32, i32, i32, f64, vp, i32, vp, i32, vp, i32, vp, i32, i32, vp], i32),
         "bb_nufft_get": ([vp, i32, vp], i32),
         "bb_nufft_stats": ([vp, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)], i32),
         "bb_status_string": ([i32], ctypes.c_char_p),
@@ -396,6 +397,18 @@ class NufftSynthesis:
         Dp, _, _, ldd = _marshal(D, np.float32, keep)
         Xp, _, _, ldx = _marshal(xyz, np.float64, keep)
         _check(_lib.bb_nufft_collect_eig(self._h, n_ant, n_eig, float(wavelength), Bp, ldb, Dp, ldd, Xp, ldx), "bb_nufft_collect_eig")
+
+    def collect(self, S, W, xyz, wavelength, n_eig, intervals, filters=None):
+        """Algorithm 3 from S, W, xyz and the intervals; filters as StandardSynthesis.collect."""
+        keep = []
+        Sp, n_beam, _, lds = _marshal(S, np.complex64, keep)
+        Wp, _, _, ldw = _marshal(W, np.complex64, keep)
+        Xp, n_ant, _, ldx = _marshal(xyz, np.float64, keep)
+        Ip, _, _, ldi = _marshal(intervals, np.float64, keep)
+        kinds = [FILTERS[f] for f in (filters or ["lsq"])]
+        arr = (ctypes.c_int * len(kinds))(*kinds)
+        _check(_lib.bb_nufft_collect(self._h, n_ant, n_beam, int(n_eig), float(wavelength), Wp, ldw, Sp, lds, Xp, ldx, Ip, ldi,
+                                     len(kinds), ctypes.cast(arr, ctypes.c_void_p)), "bb_nufft_collect")
 
     def images(self):
         out = np.empty((self.n_levels, self.n_pix), dtype=np.float32)

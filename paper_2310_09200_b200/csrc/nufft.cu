@@ -223,6 +223,9 @@ struct bb_nufft {
   struct FftPlan { cufftHandle handle; size_t work_bytes; };
   std::map<std::tuple<int, int, int>, FftPlan> plans;
   unsigned char* fft_work = nullptr; size_t fft_work_cap = 0;
+  // bb_nufft_collect (Alg. 3 from S): eigenvalues, B = W V and level weights of the current collect, device resident
+  double* lam_full = nullptr; bb_c32* B_full = nullptr; float* D_full = nullptr;
+  size_t lam_full_cap = 0, B_full_cap = 0, D_full_cap = 0;
   int64_t n_transforms = 0, max_grid = 0;
 };
 
@@ -361,7 +364,7 @@ extern "C" int bb_nufft_destroy(bb_nufft* h) {
   cudaStreamSynchronize(bb_ctx_user_stream(h->ctx));
   for (auto& kv : h->plans) cufftDestroy(kv.second.handle);
   for (auto& kv : h->dec) cudaFree(kv.second);
-  cudaFree(h->fft_work);
+  cudaFree(h->fft_work); cudaFree(h->lam_full); cudaFree(h->B_full); cudaFree(h->D_full);
   cudaFree(h->pix_dev); cudaFree(h->img); cudaFree(h->out_idx_dev); cudaFree(h->V); cudaFree(h->grid); cudaFree(h->fine);
   cudaFree(h->in_idx_dev); cudaFree(h->xyz_all_dev); cudaFree(h->inv_wl_dev); cudaFree(h->B_dev); cudaFree(h->D_dev); cudaFree(h->xyz_dev);
   bb_ctx_ref(h->ctx, -1);
@@ -588,6 +591,34 @@ extern "C" int bb_nufft_collect_eig(bb_nufft* h, int n_ant, int n_eig, double wa
   h->inv_wl_all.push_back(1.0 / wavelength);
   h->pend += 1; h->pend_n_ant = n_ant;
   return BB_OK;
+}
+
+// Algorithm 3 as the paper states it: from S, W, the antenna positions and the intervals. Lines 2-4
+// (Gram matrix, generalized eigendecomposition, N_eig largest) are the library's fp64 device glue (bb_eig), lines 6-7 the
+// level weights (bb_level_weights: interval selection and filter in one matrix D), line 8 onwards bb_nufft_collect_eig
+// (V = alpha_I diag(lambda_f) alpha_I^H per level with the beamforming folded in, B = W alpha, Eq. 17 / 21; then the NUFFT).
+// The intermediates stay on the device.
+extern "C" int bb_nufft_collect(bb_nufft* h, int n_ant, int n_beam, int n_eig, double wavelength, const bb_c32* W, int ldw,
+                                const bb_c32* S, int lds, const double* xyz, int ldxyz, const double* intervals, int ld_int,
+                                int n_filters, const int* filters) {
+  if (!h || !S || !xyz || !intervals || !filters || n_filters < 1 || n_filters > BB_MAX_FILTERS || h->n_levels % n_filters != 0)
+    return BB_EINVAL;
+  const int n_intervals = h->n_levels / n_filters;
+  if (n_ant < 1 || n_ant > 4096 || n_beam < 1 || n_beam > BB_MAX_BEAMS || n_eig < 1 || n_eig > n_beam || !(wavelength > 0.0) || lds < n_beam ||
+      ldxyz < n_ant || ld_int < n_intervals || (W && ldw < n_ant) || (!W && n_beam != n_ant))
+    return BB_EINVAL;
+  BB_CUDA(cudaSetDevice(bb_ctx_device(h->ctx)));
+  int rc;
+  if ((rc = grow(&h->lam_full, &h->lam_full_cap, (size_t)n_eig)) != BB_OK || (rc = grow(&h->B_full, &h->B_full_cap, (size_t)n_ant * n_eig)) != BB_OK ||
+      (rc = grow(&h->D_full, &h->D_full_cap, (size_t)h->n_levels * n_eig)) != BB_OK)
+    return rc;
+  // l.2-4 (+ B = W alpha). Synchronous; BB_ENOTPOSDEF / BB_ENOCONV come back directly and nothing is staged.
+  if ((rc = bb_eig(h->ctx, n_ant, n_beam, n_eig, wavelength, W, ldw, S, lds, xyz, ldxyz, h->lam_full, h->B_full, n_ant)) != BB_OK) return rc;
+  // l.5-7: D[f * n_intervals + i, k] = filter_f(lambda_k) if lambda_k lies in interval i, else 0
+  if ((rc = bb_level_weights(h->ctx, h->lam_full, n_eig, intervals, ld_int, n_intervals, n_filters, filters, h->D_full, h->n_levels)) != BB_OK)
+    return rc;
+  // l.8-9: per-level visibilities and the (staged) type-3 transform
+  return bb_nufft_collect_eig(h, n_ant, n_eig, wavelength, h->B_full, n_ant, h->D_full, h->n_levels, xyz, ldxyz);
 }
 
 extern "C" int bb_nufft_get(bb_nufft* h, int level, float* out) {

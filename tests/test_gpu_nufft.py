@@ -111,6 +111,54 @@ def test_argument_validation_and_grid_limit(bb, ctx):
     assert e.value.code == 7                                                # BB_EUNSUPPORTED: raise the partition counts
 
 
+def test_algorithm3_from_S_config1_and_filters(bb, ctx, oracle):
+    """bb_nufft_collect = Algorithm 3 as printed: Gram, generalized eigendecomposition, N_eig largest,
+    intervals and filters, V per level, NUFFT. Reference: the oracle's Algorithm 1 from the same S (the two synthesizers
+    compute the same image, Eq. 15/20 vs Eq. 17-19/21, pinned on the CPU side), with one LSQ filter and with (STD, LSQ)."""
+    from paper_2310_09200_b200 import workloads
+    w = workloads.make_workload(1)
+    ci = w.collect_inputs(0)
+    pix = w.pixels()
+    lam, _ = oracle.eig_stage(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig)
+    iv = workloads.choose_intervals(lam, w.cfg.n_levels)
+    ref = oracle.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, pix)
+    h = bb.NufftSynthesis(ctx, pix, w.cfg.n_levels, eps=1e-6)
+    h.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv)
+    h.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv)          # two time steps staged, one set of transforms
+    assert_parity(h.images(), 2 * ref, "Algorithm 3 from S, config 1")
+    ref2 = oracle.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, pix, filt=("std", "lsq"))
+    h2 = bb.NufftSynthesis(ctx, pix, 2 * w.cfg.n_levels, eps=1e-6)
+    h2.collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, filters=["std", "lsq"])
+    assert_parity(h2.images(), ref2, "Algorithm 3 from S, config 1, filters (std, lsq)")
+    with pytest.raises(bb.BluebildError):                                               # 3 levels cannot hold 2 filters x 2 intervals
+        bb.NufftSynthesis(ctx, pix, 3, eps=1e-6).collect(ci["S"], ci["W"], ci["xyz"], ci["wavelength"], w.cfg.n_eig, iv, filters=["std", "lsq"])
+    # a Gram matrix that is not positive definite (all antennas at the same place: all ones) is reported by the call itself
+    xyz_bad = ci["xyz"].copy()
+    xyz_bad[:] = xyz_bad[0]
+    with pytest.raises(bb.BluebildError) as e:
+        h.collect(ci["S"], ci["W"], np.asfortranarray(xyz_bad), ci["wavelength"], w.cfg.n_eig, iv)
+    assert e.value.code == 4
+    assert_parity(h.images(), 2 * ref, "images unchanged by the refused collect")
+
+
+def test_algorithm3_from_S_config3_three_collects(bb, ctx, oracle):
+    """Three collects of BASELINE config 3 (epochs 0, 50, 99) through bb_nufft_collect from S, 64 x 64 input cells, against the
+    oracle's Algorithm 1 on the every-16th pixel subset (the device glue's eigenpairs, not the oracle's, feed the NUFFT)."""
+    from paper_2310_09200_b200 import workloads
+    from helpers import intervals_for
+    w = workloads.make_workload(3)
+    c = w.cfg
+    iv = intervals_for(oracle, workloads, w, [0, 50, 99])
+    sub = w.sample_pixels(16)
+    ref = np.zeros((c.n_levels, sub.size))
+    h = bb.NufftSynthesis(ctx, w.pixels(), c.n_levels, eps=1e-5, n_part_in=64, n_part_out=1)
+    for n in (0, 50, 99):
+        r = w.collect_inputs(n)
+        oracle.collect(r["S"], r["W"], r["xyz"], r["wavelength"], c.n_eig, iv, w.pixels(sub), img=ref)
+        h.collect(r["S"], r["W"], r["xyz"], r["wavelength"], c.n_eig, iv)
+    assert_parity(h.images()[:, sub], ref, "Algorithm 3 from S, config 3")
+
+
 def test_a_refused_flush_leaves_the_images_untouched(bb, ctx):
     """the grid limit is checked for ALL (input cell, output cell) pairs before any of them is transformed. Seven
     antennas within 50 m and one 570 km away, 2 x 2 input cells: the cells that hold only short baselines need tiny grids,
