@@ -290,7 +290,8 @@ int bb_nufft_plan(int64_t n_pix, const double* pix, int64_t ld_pix, int n_ant, c
                   double eps, int n_part_in, int n_part_out, int64_t* n_transforms, int64_t* max_grid_points,
                   double* sum_grid_points, double* nonempty_input_cells);
 
-/* ---- launch-shape query (host only, no device needed) ---------------------------------------------
+/* ---- DIAGNOSTICS: launch-shape query (host only, no device needed). Like bb_synth_launches it follows no passage of
+ * the paper: both exist so that tests and bench.py can check and count what the library launches. -------------------
  * Number of collect ranges a synthesizer launch over n_collects queued collects is split into on a GPU with sm_count
  * SMs: 1 = one CTA per pixel tile handles all collects; > 1 for small images whose tile count would leave most of a
  * wave of SMs empty (the ranges' level sums are added in a fixed order). Returns 0 on invalid arguments. */
